@@ -1,0 +1,88 @@
+"""Helpers for the oracle pin tests (no method arithmetic beyond textbook closed forms)."""
+import numpy as np
+
+from paper_0910_5547_b200 import workloads as wl
+
+
+def slab_hierarchy(nblocks_x, axis=0, periodic=True):
+    """nblocks_x patches along `axis`, one patch thick in the other two (periodic there)."""
+    nb = [1, 1, 1]
+    nb[axis] = nblocks_x
+    bc = [0] * 6
+    if not periodic:
+        bc[2 * axis] = bc[2 * axis + 1] = 1
+    # box = extent along x, chosen so that dx = 1/(16 nblocks_x) whatever the axis
+    return wl.build_hierarchy(tuple(nb), (), tuple(bc), box=nb[0] / float(nblocks_x), order="linear"), nb
+
+
+def slab_dx(nblocks_x):
+    return 1.0 / (16 * nblocks_x)
+
+
+def exact_sod(x, t, gamma=1.4, left=(1.0, 0.0, 1.0), right=(0.125, 0.0, 0.1), x0=0.5):
+    """Exact Riemann solution (rho, u, p) for a left-rarefaction / right-shock pattern.
+    Textbook (Toro ch. 4): Newton iteration on the pressure function."""
+    rl, ul, pl = left
+    rr, ur, pr = right
+    g = gamma
+    cl, cr = np.sqrt(g * pl / rl), np.sqrt(g * pr / rr)
+
+    def f(p, r, pk, ck):
+        if p > pk:  # shock
+            A, B = 2.0 / ((g + 1) * r), (g - 1) / (g + 1) * pk
+            return (p - pk) * np.sqrt(A / (p + B))
+        return 2 * ck / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1)
+
+    lo, hi = 1e-8, 10.0
+    for _ in range(200):  # bisection: robust, no derivative needed
+        mid = 0.5 * (lo + hi)
+        if f(mid, rl, pl, cl) + f(mid, rr, pr, cr) + ur - ul > 0:
+            hi = mid
+        else:
+            lo = mid
+    ps = 0.5 * (lo + hi)
+    us = 0.5 * (ul + ur) + 0.5 * (f(ps, rr, pr, cr) - f(ps, rl, pl, cl))
+    rsl = rl * (ps / pl) ** (1 / g)                      # behind the rarefaction
+    rsr = rr * ((ps / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * ps / pr + 1))  # behind the shock
+    S = ur + cr * np.sqrt((g + 1) / (2 * g) * ps / pr + (g - 1) / (2 * g))
+    csl = cl * (ps / pl) ** ((g - 1) / (2 * g))
+    xi = (x - x0) / t
+    rho = np.empty_like(x); u = np.empty_like(x); p = np.empty_like(x)
+    for n, s in enumerate(xi):
+        if s < ul - cl:
+            rho[n], u[n], p[n] = rl, ul, pl
+        elif s < us - csl:
+            c = 2 / (g + 1) * (cl + (g - 1) / 2 * (ul - s))
+            u[n] = 2 / (g + 1) * (cl + (g - 1) / 2 * ul + s)
+            rho[n] = rl * (c / cl) ** (2 / (g - 1))
+            p[n] = pl * (c / cl) ** (2 * g / (g - 1))
+        elif s < us:
+            rho[n], u[n], p[n] = rsl, us, ps
+        elif s < S:
+            rho[n], u[n], p[n] = rsr, us, ps
+        else:
+            rho[n], u[n], p[n] = rr, ur, pr
+    return rho, u, p, dict(ps=ps, us=us, rsl=rsl, rsr=rsr, S=S)
+
+
+def run_to(o, t_end, cfl, max_steps=100000):
+    """Advance the oracle to exactly t_end (last step shortened)."""
+    t, n = 0.0, 0
+    while t < t_end * (1 - 1e-12) and n < max_steps:
+        dt = o.cfl_dt(0, 0, cfl)
+        if t + dt > t_end:
+            dt = t_end - t
+        o.advance(cfl, dt)
+        t += dt
+        n += 1
+    return n
+
+
+def norm_err(a, b):
+    """S14: per-variable max|a-b| / max|b| (0/0 = 0)."""
+    out = []
+    for v in range(b.shape[1]):
+        d = np.abs(a[:, v] - b[:, v]).max()
+        s = np.abs(b[:, v]).max()
+        out.append(0.0 if d == 0 else d / s if s > 0 else np.inf)
+    return np.array(out)
