@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s per full RK2 step of the AMR finite-volume hot path on B200.
+
+One "step" = one pass of the whole hot path over one level/hierarchy: CFL reduction, ghost
+fill, RK stage 1, ghost fill, RK stage 2 (plus restriction/refluxing on AMR workloads).
+Default workload: BASELINE.json configs[4] (512^3 uniform periodic Euler stress test, 32768
+patches of 16^3), the configuration the metric is quoted on.  Inputs are seeded and synthetic
+(paper_0910_5547_b200/workloads.py).  Prints ONE JSON line on rank 0.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--impl ours|reference]
+                  [--workload cfg5|cfg2|cfg4|cfg3] [--size S] [--halo 0|1]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_0910_5547_b200 import workloads as wl  # noqa: E402
+
+# dram__bytes_read.sum + dram__bytes_write.sum per rk_stage launch from the `ncu --set full`
+# capture summarised under profiles/ (None until a capture of this configuration exists).
+NCU_TRAFFIC = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic.json")) as _f:
+        NCU_TRAFFIC = json.load(_f)
+except Exception:
+    pass
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg5", "cfg2", "cfg4", "cfg3"])
+    ap.add_argument("--size", type=int, default=0, help="cells per side (default: the config's own size)")
+    ap.add_argument("--halo", type=int, default=1, help="1: rk_stage reads sibling interiors directly")
+    ap.add_argument("--kernel", type=int, default=1)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    return ap.parse_args()
+
+
+WORKLOADS = {
+    "cfg5": dict(size=512, gamma=1.4, nv=5, cfl=0.3, name="cfg5_euler_stress_512^3_periodic"),
+    "cfg2": dict(size=256, gamma=5.0 / 3.0, nv=5, cfl=0.3, name="cfg2_kelvin_helmholtz_256^3_periodic"),
+    "cfg4": dict(size=128, gamma=5.0 / 3.0, nv=8, cfl=0.3, name="cfg4_mhd_turbulence_128^3_periodic"),
+    "cfg3": dict(size=64, gamma=1.4, nv=5, cfl=0.3, name="cfg3_sedov_amr_64^3+4levels"),
+}
+
+
+def make_workload(name, size, seed_shift=0):
+    """Returns (hierarchy, U[npatch][nv][16][16][16] float64, cell-updates per coarse step)."""
+    w = WORKLOADS[name]
+    n = size or w["size"]
+    if name == "cfg3":
+        h = wl.ball_hierarchy(n // 16, 5, bc=(1,) * 6)
+        U = wl.sedov_hierarchy_state(h, gamma=w["gamma"])
+        upd = sum(int((h["level"] == l).sum()) * 4096 * (1 << l) for l in range(h["nlevels"]))
+        return h, U, upd
+    h = wl.uniform_hierarchy(n // 16, periodic=True)
+    if name == "cfg5":
+        G = wl.stress_global(n, gamma=w["gamma"], seed=20005 + seed_shift)
+    elif name == "cfg2":
+        G = wl.kelvin_helmholtz_global(n, gamma=w["gamma"], seed=20002 + seed_shift)
+    else:
+        G = wl.mhd_turbulence_global(n, gamma=w["gamma"], seed=20004 + seed_shift)
+    U = wl.split_global(h, G)
+    del G
+    return h, U, n ** 3
+
+
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        for line in self.f:
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 9:
+                continue
+            try:
+                sm.append(float(t[1])); mx.append(float(t[2])); pw.append(float(t[3]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), t[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=float(max(pw)))
+        return out
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def cpu_oracle_rate(name, size, seconds=10.0, dtype="f64"):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload:
+    a contiguous 64^3 block (4x4x4 patches) of the workload's initial data, periodic on the
+    block; full RK2 steps until `seconds` of wall time have elapsed (at least 2 steps)."""
+    import oracle
+    w = WORKLOADS[name]
+    cores = os.cpu_count() or 1
+    if name == "cfg3":
+        h, U, upd = make_workload("cfg3", size)
+        sample = "whole cfg3 hierarchy (%d patches), coarse steps" % len(h["level"])
+    else:
+        h, U, upd = make_workload(name, 64)
+        sample = "64^3 block (64 patches) generated by the same recipe, periodic, full RK2 steps"
+    o = oracle.Oracle(h, w["gamma"], w["nv"], bits=64, threads=cores)
+    o.upload(0, U)
+    o.advance(w["cfl"])  # warm-up (page-in)
+    t0 = time.perf_counter()
+    n = 0
+    while n < 2 or time.perf_counter() - t0 < seconds:
+        o.advance(w["cfl"])
+        n += 1
+    dt = time.perf_counter() - t0
+    return upd * n / dt, cores, sample + ", %d steps in %.1f s" % (n, dt), dt / n
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = WORKLOADS[args.workload]
+    rate, cores, sample, per_step = cpu_oracle_rate(args.workload, args.size, seconds=max(5.0, 2.0 * args.steps))
+    line = {
+        "impl": "reference", "metric": "cell-updates/sec per RK2 step", "value": rate, "unit": "cell-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w["name"], "note": "CPU oracle (oracle/amr_oracle.cpp) on a bounded sample"},
+        "cpu_baseline": {"value": rate, "unit": "cell-updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    from paper_0910_5547_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the amrhydro path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = WORKLOADS[args.workload]
+    nv, gamma, cfl = w["nv"], w["gamma"], w["cfl"]
+    h, U, upd_per_step = make_workload(args.workload, args.size, seed_shift=rank)
+    npatch = len(h["level"])
+    single = h["nlevels"] == 1
+    esz = 8 if args.dtype == "f64" else 4
+    npdt = np.float64 if args.dtype == "f64" else np.float32
+    g = binding.AmrHydro(h, gamma, nv, dtype=args.dtype, halo=args.halo, kernel=args.kernel, device="cuda:%d" % local)
+    host_in = torch.empty((npatch, nv, 16, 16, 16), dtype=torch.float64 if esz == 8 else torch.float32, pin_memory=True)
+    host_in.numpy()[...] = U.astype(npdt, copy=False)
+    del U
+    g.upload_ptr(0, 0, npatch, host_in.data_ptr())
+    g.sync()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    stage_ev = []
+
+    def step(record=False):
+        if single:
+            dt = g.cfl_dt(0, 0, cfl)
+            g.fill_ghosts(0, 0)
+            if record:
+                e0, e1, e2, e3 = ev(), ev(), ev(), ev()
+                e0.record()
+            g.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
+            if record:
+                e1.record()
+            g.fill_ghosts(0, 1)
+            if record:
+                e2.record()
+            g.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+            if record:
+                e3.record()
+                stage_ev.append((e0, e1, e2, e3))
+        else:
+            g.advance(cfl)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    g.get_counter(binding.CNT_LAUNCHES, reset=True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0, t1 = ev(), ev()
+    t0.record()
+    for _ in range(args.steps):
+        step(record=True)
+    t1.record()
+    barrier()
+    ms = t0.elapsed_time(t1)
+    clocks = sampler.stop() if sampler else {}
+    launches = g.get_counter(binding.CNT_LAUNCHES)
+    if dist is not None:
+        tt = torch.tensor([ms], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    ms_per_step = ms / args.steps
+    value = upd_per_step * world * args.steps / (ms * 1e-3)
+
+    # finiteness of the state after the timed run (S4 warning): sample the first patches
+    chk = g.download(0, 0, min(npatch, 64))
+    finite = bool(np.isfinite(chk).all())
+
+    # roofline of the dominant kernel (rk_stage): algorithmic bytes / measured launch time
+    peak, peak_src = peaks()
+    roof = None
+    if stage_ev:
+        s1 = float(np.mean([a.elapsed_time(b) for a, b, _, _ in stage_ev]))
+        s2 = float(np.mean([c.elapsed_time(d) for _, _, c, d in stage_ev]))
+        cells = npatch * 4096
+        b1, b2 = 2 * nv * esz * cells, 3 * nv * esz * cells       # stage 1: read U write U1; stage 2: + read Un
+        avg_ms = 0.5 * (s1 + s2)
+        ach = 0.5 * (b1 + b2) / (avg_ms * 1e-3) / 1e9
+        key = "%s_%s" % (args.workload, args.dtype)
+        roof = {"bound": "hbm", "kernel": "k_rk_stage_tile" if args.kernel == 1 else "k_rk_stage_ref",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": NCU_TRAFFIC.get(key), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": 0.5 * (b1 + b2),
+                "stage1": {"ms": s1, "GB/s": b1 / (s1 * 1e-3) / 1e9, "bytes_per_cell": 2 * nv * esz},
+                "stage2": {"ms": s2, "GB/s": b2 / (s2 * 1e-3) / 1e9, "bytes_per_cell": 3 * nv * esz},
+                "share_of_step": (s1 + s2) / ms_per_step,
+                "frac_of_nominal_8TBs": ach / 8000.0}
+
+    # end to end through the C ABI with host buffers (H2D of all interiors, one step, D2H)
+    e2e = None
+    if not args.no_e2e:
+        host_out = torch.empty_like(host_in)
+        hb = npatch * nv * 4096 * esz
+        g.advance_host(cfl, 0.0, 1, host_in.data_ptr(), host_out.data_ptr())      # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            g.advance_host(cfl, 0.0, 1, host_in.data_ptr(), host_out.data_ptr())
+        torch.cuda.synchronize()
+        el = time.perf_counter() - t0
+        if dist is not None:
+            tt = torch.tensor([el], device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            el = float(tt.item())
+        e2e = {"value": upd_per_step * world * args.e2e_steps / el, "unit": "cell-updates/s",
+               "h2d_bytes_per_step": hb, "d2h_bytes_per_step": hb, "steps": args.e2e_steps,
+               "api": "amrhydro_advance_host (pinned host buffers)"}
+        finite = finite and bool(np.isfinite(host_out.numpy()[:8]).all())
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        rate, cores, sample, _ = cpu_oracle_rate(args.workload, args.size)
+        cpu = {"value": rate, "unit": "cell-updates/s", "cores": cores, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        line = {
+            "metric": "cell-updates/sec per RK2 step", "value": value, "unit": "cell-updates/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+            "data": "synthetic",
+            "config": {"workload": w["name"], "patches": npatch, "cells": npatch * 4096, "nvars": nv,
+                       "cfl": cfl, "halo": "direct sibling reads" if args.halo else "materialised ghosts",
+                       "l2_policy": "working set (%.1f GB per slot) far exceeds the 126 MB L2" % (npatch * nv * 4096 * esz / 1e9)
+                       if npatch * nv * 4096 * esz > 4 * 126e6 else "working set fits L2 (small config)",
+                       "parallelism": "replicas, one per GPU" if world > 1 else "single GPU"},
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks, "finite": finite,
+            "paper_context": "paper reports 8-10x vs one 3 GHz core on a Quadro FX 5600, fp32 (PAPER.md:274)",
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    if not finite:
+        raise SystemExit("non-finite state after the timed run")
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

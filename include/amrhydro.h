@@ -1,0 +1,154 @@
+/* amrhydro.h -- C ABI of the B200 (sm_100a) block-AMR finite-volume hot path.
+ *
+ * Method: Wang, Abel & Kaehler, "Adaptive Mesh Fluid Simulations on GPU", arXiv:0910.5547.
+ * Citations "PAPER.md:<line>" refer to the extracted paper text; "S<n>/G<n>" to the readings
+ * listed in DESIGN.md where the paper is silent or garbled.
+ *
+ * Conventions
+ *  - Plain C symbols, opaque handle, no exceptions, no printing.  Every call except
+ *    create/destroy/last_error/pool_bytes returns an int status: 0 = OK, negative = error
+ *    (see AMRHYDRO_E*); amrhydro_last_error(h) then returns a static/handle-owned string.
+ *  - All kernels are enqueued on the CUDA stream given to amrhydro_bind_pool and are
+ *    asynchronous.  Calls that return host data (cfl_dt, download_*, advance, counters)
+ *    synchronise that stream.
+ *  - Ownership: the caller (PyTorch) owns the pool allocation and the stream; the library
+ *    borrows them.  The library owns the device copy of the descriptor table, the flux
+ *    registers, the boundary-flux scratch, the reduction scratch and a host<->device staging
+ *    buffer; amrhydro_destroy frees them.
+ *  - Pointers: `dev_*` are device pointers, `host_*` are host pointers (pageable or pinned).
+ *  - Geometry: patch interior 16^3, 2 ghost zones, refinement ratio 2, cubic cells,
+ *    dx_l = dx0 / 2^l.  nvars = 5 (Euler: rho, rho vx, rho vy, rho vz, rho E; PAPER.md:57
+ *    Eq. 2) or 8 (ideal MHD: ... rho E + B^2/2, Bx, By, Bz; Eq. 14 without psi).
+ *  - Host-side patch data is always "interior" layout [var][16][16][16] (x fastest) of the
+ *    element type selected by AMRHYDRO_OPT_DTYPE.  The pool's internal (padded, aligned)
+ *    layout is private.
+ *  - Slots: by convention 0 = A (U^n -> U^{n+1}), 1 = B (U^(1)), 2 = C (U^n of a level with
+ *    children); the primitive calls take explicit slot numbers.
+ *  - There is no CPU fallback: every call fails with AMRHYDRO_ECUDA when no device is usable.
+ */
+#ifndef AMRHYDRO_H
+#define AMRHYDRO_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AMRHYDRO_OK 0
+#define AMRHYDRO_EINVAL (-1)    /* bad argument                                   */
+#define AMRHYDRO_ENOMEM (-2)    /* pool too small / allocation failed              */
+#define AMRHYDRO_ECUDA (-3)     /* CUDA runtime error (text in last_error)         */
+#define AMRHYDRO_ESTATE (-4)    /* call out of order (no pool / no hierarchy)      */
+#define AMRHYDRO_ENONFINITE (-5)/* NaN/inf/zero signal speed in cfl_dt / advance   */
+
+/* options (amrhydro_set_option); only before amrhydro_bind_pool unless noted */
+#define AMRHYDRO_OPT_DTYPE 1      /* 32 or 64 (default 64): element type of pool and host data   */
+#define AMRHYDRO_OPT_THETA 2      /* limiter parameter of Eq. 9-10, 0..2 (default 1.5, S1); any time */
+#define AMRHYDRO_OPT_RHO_FLOOR 3  /* S11, default 1e-30; any time                                  */
+#define AMRHYDRO_OPT_EINT_FLOOR 4 /* S11, default 1e-30; any time                                  */
+#define AMRHYDRO_OPT_KERNEL 5     /* rk_stage variant: 0 = reference one-thread-per-cell kernel,
+                                     1 = z-marching shared-memory kernel (default); any time      */
+#define AMRHYDRO_OPT_HALO 6       /* 0 = rk_stage reads materialised ghost zones (default);
+                                     1 = rk_stage reads sibling interiors directly, fill_ghosts
+                                     then only writes coarse-fine / physical faces; any time      */
+
+/* counters (amrhydro_get_counter) */
+#define AMRHYDRO_CNT_LAUNCHES 1   /* kernels launched by this handle since create / last reset */
+#define AMRHYDRO_CNT_FLOOR_HITS 2 /* cells/states where a floor of S11 was applied (rk_stage, cfl) */
+
+#define AMRHYDRO_BC_PERIODIC 0    /* handled by the neighbour table */
+#define AMRHYDRO_BC_OUTFLOW 1     /* zero-gradient (S5)             */
+
+#define AMRHYDRO_NBR_COARSE_FINE (-1)
+#define AMRHYDRO_NBR_PHYSICAL (-2)
+
+typedef struct amrhydro amrhydro_t;
+
+/* One row of the patch-descriptor table (128 bytes).  Patches must be sorted by level.
+ * origin: index of the first interior cell on the patch's own level (multiple of 16).
+ * parent: patch id on level-1 whose octant this patch refines (-1 on level 0).
+ * nbr[r], r = (dz+1)*9 + (dy+1)*3 + (dx+1): id of the same-level patch at block offset
+ * (dx,dy,dz) (periodic wrap is expressed here), AMRHYDRO_NBR_COARSE_FINE or
+ * AMRHYDRO_NBR_PHYSICAL; nbr[13] is ignored. */
+typedef struct amrhydro_patch_desc {
+  int level;
+  int origin[3];
+  int parent;
+  int nbr[27];
+} amrhydro_patch_desc;
+
+/* Create a solver context.  gamma: adiabatic index of Eq. 6, > 1.
+ * nvars in {5, 8}; patch_dim must be 16 and nghost 2 (BASELINE.json north_star; the stencil
+ * i-2..i+1 of PAPER.md:104).  Returns NULL on a bad argument or when no CUDA device exists. */
+amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost);
+void amrhydro_destroy(amrhydro_t *h);
+const char *amrhydro_last_error(const amrhydro_t *h);
+
+int amrhydro_set_option(amrhydro_t *h, int key, double value);
+int amrhydro_get_counter(amrhydro_t *h, int key, long long *value_out, int reset);
+
+/* Bytes the caller must allocate for `nslots` copies of `max_patches` padded patches. */
+size_t amrhydro_pool_bytes(const amrhydro_t *h, int max_patches, int nslots);
+/* Borrow the pool (device pointer, 256-byte aligned) and the stream (cudaStream_t as void*,
+ * NULL = legacy default stream).  The pool is zero-filled asynchronously. */
+int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patches, int nslots,
+                       void *cuda_stream);
+/* Copy and validate the descriptor table (host memory, owned by the caller).  dx0: level-0
+ * cell width; bc[6]: AMRHYDRO_BC_* for x-lo, x-hi, y-lo, y-hi, z-lo, z-hi.  Allocates and
+ * zeroes the flux registers when nlevels > 1. */
+int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *host_tbl, int npatches,
+                           int nlevels, double dx0, const int *bc);
+
+/* Interior data of patches [first, first+count) of one slot, host layout
+ * [count][var][16][16][16].  Upload stages through the library's device buffer in chunks;
+ * pinned host memory makes the copies asynchronous. */
+int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *host_interior);
+int amrhydro_download(amrhydro_t *h, int slot, int first, int count, void *host_interior);
+/* Debug/test: padded box [var][20][20][20] of one patch, and its flux registers
+ * [6 faces][var][8][8] (fine side, coarse side), as doubles. */
+int amrhydro_download_padded(amrhydro_t *h, int slot, int patch, double *host_padded);
+int amrhydro_download_registers(amrhydro_t *h, int patch, double *host_fine, double *host_coarse);
+
+/* a1: dt = cfl * dx_level / max over interior cells and d of (|v_d| + c_d), c = sound speed
+ * (S2) or fast magnetosonic speed along d (S3).  S4; the paper gives no CFL formula.
+ * Synchronises.  AMRHYDRO_ENONFINITE if the maximum is NaN, inf or 0.  smax_out may be NULL. */
+int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_out, double *smax_out);
+
+/* a2: fill the ghost zones of every patch of `level` in `slot` (S5): same-level copy where
+ * nbr >= 0; conservative limited-linear prolongation (S6) of (1-alpha)*parent_old_slot +
+ * alpha*parent_new_slot (S7) where nbr == -1; zero-gradient outflow where nbr == -2. */
+int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int parent_old_slot,
+                         int parent_new_slot, double alpha);
+
+/* a3-a6: one method-of-lines stage on every patch of `level` (PAPER.md:79 Eq. 7, :94-98
+ * Eq. 8): U_out = a*U_base + b*(U_in + dt*L(U_in)), L from primitive recovery, PLM with the
+ * theta-minmod limiter (Eq. 9-11, G1) and the single-speed HLL flux (Eq. 12, G2, G6).
+ * slot_out may equal slot_base, must differ from slot_in.  flux_weight w != 0 accumulates
+ * w*dt*F on coarse-fine faces into the flux registers (S10). */
+int amrhydro_rk_stage(amrhydro_t *h, int level, int slot_in, int slot_base, int slot_out,
+                      double a, double b, double dt, double flux_weight);
+
+/* a7: each covered cell of level fine_level-1 := mean of its 8 fine cells (S8). */
+int amrhydro_restrict(amrhydro_t *h, int fine_level, int fine_slot, int coarse_slot);
+/* a8: correct the uncovered coarse cells next to level coarse_level+1 patches with the
+ * accumulated flux mismatch, then zero those registers (S10). */
+int amrhydro_reflux(amrhydro_t *h, int coarse_level, int slot);
+
+int amrhydro_copy_slot(amrhydro_t *h, int level, int src_slot, int dst_slot);
+
+/* Host-side driver (bookkeeping only): one coarse step of the whole hierarchy with
+ * ratio-2 subcycling (S9), slots 0/1/2 as above.  dt_fixed > 0 overrides the CFL step
+ * dt0 = cfl*dx0 / max_l S_max,l (S4).  Synchronises once (for dt) unless dt_fixed > 0. */
+int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out);
+/* End-to-end variant with host buffers: upload all interiors into slot 0, `nsteps` coarse
+ * steps, download slot 0.  host_in/host_out: [npatches][var][16][16][16]. */
+int amrhydro_advance_host(amrhydro_t *h, double cfl, double dt_fixed, int nsteps,
+                          const void *host_in, void *host_out, double *dt_last_out);
+
+int amrhydro_sync(amrhydro_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMRHYDRO_H */

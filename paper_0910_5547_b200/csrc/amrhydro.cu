@@ -1,0 +1,557 @@
+// amrhydro.cu -- host side of the C ABI declared in include/amrhydro.h: handle, descriptor
+// table, launches, and the subcycling driver (host bookkeeping only; every arithmetic step of
+// the path runs in the kernels).  There is no CPU fallback anywhere in this file.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <type_traits>
+#include <vector>
+
+#include "../../include/amrhydro.h"
+#include "kernels_level.cuh"
+#include "layout.cuh"
+#include "physics.cuh"
+#include "rk_stage_ref.cuh"
+#include "rk_stage_tile.cuh"
+
+using namespace amr;
+
+static_assert(sizeof(amrhydro_patch_desc) == 128 && sizeof(Desc) == 128, "descriptor row is 128 bytes");
+
+struct amrhydro {
+  double gamma = 1.4;
+  int nv = 5, bits = 64;
+  double theta = 1.5, rho_floor = 1e-30, e_floor = 1e-30;
+  int kernel = 1, halo = 0;
+  void *pool = nullptr;
+  size_t pool_bytes = 0;
+  int maxp = 0, nslots = 0;
+  cudaStream_t stream = nullptr;
+  bool bound = false;
+  int np = 0, nlev = 0;
+  double dx0 = 1.0;
+  int bc[6] = {0, 0, 0, 0, 0, 0};
+  std::vector<amrhydro_patch_desc> tbl;
+  std::vector<int> child, octant, lev_first, lev_count;
+  Desc *d_desc = nullptr;
+  int *d_child = nullptr, *d_octant = nullptr;
+  void *d_Rf = nullptr, *d_Rc = nullptr, *d_bflux = nullptr;
+  size_t bflux_patches = 0;
+  unsigned long long *d_scalars = nullptr;  // [0] smax bits, [1] floor hits
+  void *d_stage = nullptr;
+  size_t stage_bytes = 0;
+  long long launches = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(amrhydro *h, int code, const std::string &msg) {
+  if (h) h->err = msg;
+  return code;
+}
+#define CUDA_TRY(h, expr)                                                                   \
+  do {                                                                                      \
+    cudaError_t e_ = (expr);                                                                \
+    if (e_ != cudaSuccess)                                                                  \
+      return fail(h, AMRHYDRO_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));   \
+  } while (0)
+#define LAUNCH_CHECK(h)                                                                     \
+  do {                                                                                      \
+    ++(h)->launches;                                                                        \
+    cudaError_t e_ = cudaGetLastError();                                                    \
+    if (e_ != cudaSuccess) return fail(h, AMRHYDRO_ECUDA, std::string("launch: ") + cudaGetErrorString(e_)); \
+  } while (0)
+
+template <class F> int dispatch(amrhydro *h, F &&f) {
+  if (h->bits == 64) {
+    if (h->nv == 5) return f(double(0), std::integral_constant<int, 5>());
+    return f(double(0), std::integral_constant<int, 8>());
+  }
+  if (h->nv == 5) return f(float(0), std::integral_constant<int, 5>());
+  return f(float(0), std::integral_constant<int, 8>());
+}
+
+template <typename T> Params<T> make_params(const amrhydro *h) {
+  Params<T> P;
+  P.gamma = T(h->gamma);
+  P.gm1 = T(h->gamma - 1.0);
+  P.gg1 = T(h->gamma * (h->gamma - 1.0));
+  P.theta = T(h->theta);
+  P.rho_floor = T(h->rho_floor);
+  P.e_floor = T(h->e_floor);
+  return P;
+}
+template <typename T> Pool<T> make_pool(const amrhydro *h) { return Pool<T>{(T *)h->pool, h->maxp, h->nv}; }
+
+size_t elem(const amrhydro *h) { return h->bits == 64 ? 8 : 4; }
+size_t vs(const amrhydro *h) { return h->bits == 64 ? Layout<double>::VS : Layout<float>::VS; }
+
+int check_ready(amrhydro *h, bool need_hier = true) {
+  if (!h) return AMRHYDRO_EINVAL;
+  if (!h->bound) return fail(h, AMRHYDRO_ESTATE, "no pool bound");
+  if (need_hier && h->np == 0) return fail(h, AMRHYDRO_ESTATE, "no hierarchy set");
+  return 0;
+}
+int check_level(amrhydro *h, int level) {
+  if (level < 0 || level >= h->nlev) return fail(h, AMRHYDRO_EINVAL, "level out of range");
+  return 0;
+}
+int check_slot(amrhydro *h, int s) {
+  if (s < 0 || s >= h->nslots) return fail(h, AMRHYDRO_EINVAL, "slot out of range");
+  return 0;
+}
+
+int ensure_stage(amrhydro *h, size_t bytes) {
+  if (h->stage_bytes >= bytes) return 0;
+  if (h->d_stage) cudaFree(h->d_stage);
+  h->d_stage = nullptr;
+  h->stage_bytes = 0;
+  CUDA_TRY(h, cudaMalloc(&h->d_stage, bytes));
+  h->stage_bytes = bytes;
+  return 0;
+}
+
+void free_hierarchy(amrhydro *h) {
+  cudaFree(h->d_desc); cudaFree(h->d_child); cudaFree(h->d_octant);
+  cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux);
+  h->d_desc = nullptr; h->d_child = h->d_octant = nullptr;
+  h->d_Rf = h->d_Rc = h->d_bflux = nullptr;
+  h->bflux_patches = 0;
+  h->np = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) {
+  if (!(gamma > 1.0) || (nvars != 5 && nvars != 8) || patch_dim != NI || nghost != NG) return nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return nullptr;   // no CPU fallback
+  amrhydro *h = new amrhydro;
+  h->gamma = gamma;
+  h->nv = nvars;
+  if (cudaMalloc(&h->d_scalars, 2 * sizeof(unsigned long long)) != cudaSuccess) { delete h; return nullptr; }
+  cudaMemset(h->d_scalars, 0, 2 * sizeof(unsigned long long));
+  return h;
+}
+
+void amrhydro_destroy(amrhydro_t *h) {
+  if (!h) return;
+  if (h->bound) cudaStreamSynchronize(h->stream);
+  free_hierarchy(h);
+  cudaFree(h->d_scalars);
+  cudaFree(h->d_stage);
+  delete h;
+}
+
+const char *amrhydro_last_error(const amrhydro_t *h) { return h ? h->err.c_str() : "null handle"; }
+
+int amrhydro_set_option(amrhydro_t *h, int key, double value) {
+  if (!h) return AMRHYDRO_EINVAL;
+  switch (key) {
+    case AMRHYDRO_OPT_DTYPE:
+      if (h->bound) return fail(h, AMRHYDRO_ESTATE, "dtype must be set before bind_pool");
+      if (value != 32 && value != 64) return fail(h, AMRHYDRO_EINVAL, "dtype must be 32 or 64");
+      h->bits = int(value);
+      return 0;
+    case AMRHYDRO_OPT_THETA:
+      if (!(value >= 0.0 && value <= 2.0)) return fail(h, AMRHYDRO_EINVAL, "theta must lie in [0,2]");
+      h->theta = value;
+      return 0;
+    case AMRHYDRO_OPT_RHO_FLOOR: h->rho_floor = value; return 0;
+    case AMRHYDRO_OPT_EINT_FLOOR: h->e_floor = value; return 0;
+    case AMRHYDRO_OPT_KERNEL:
+      if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0 or 1");
+      h->kernel = int(value);
+      return 0;
+    case AMRHYDRO_OPT_HALO:
+      if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "halo must be 0 or 1");
+      h->halo = int(value);
+      return 0;
+  }
+  return fail(h, AMRHYDRO_EINVAL, "unknown option");
+}
+
+int amrhydro_get_counter(amrhydro_t *h, int key, long long *out, int reset) {
+  if (!h || !out) return AMRHYDRO_EINVAL;
+  if (key == AMRHYDRO_CNT_LAUNCHES) {
+    *out = h->launches;
+    if (reset) h->launches = 0;
+    return 0;
+  }
+  if (key == AMRHYDRO_CNT_FLOOR_HITS) {
+    unsigned long long v = 0;
+    CUDA_TRY(h, cudaMemcpyAsync(&v, h->d_scalars + 1, sizeof(v), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    *out = (long long)v;
+    if (reset) CUDA_TRY(h, cudaMemsetAsync(h->d_scalars + 1, 0, sizeof(v), h->stream));
+    return 0;
+  }
+  return fail(h, AMRHYDRO_EINVAL, "unknown counter");
+}
+
+size_t amrhydro_pool_bytes(const amrhydro_t *h, int max_patches, int nslots) {
+  if (!h || max_patches <= 0 || nslots <= 0) return 0;
+  return size_t(nslots) * size_t(max_patches) * size_t(h->nv) * vs(h) * elem(h);
+}
+
+int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patches, int nslots, void *stream) {
+  if (!h || !dev_pool) return AMRHYDRO_EINVAL;
+  size_t need = amrhydro_pool_bytes(h, max_patches, nslots);
+  if (need == 0) return fail(h, AMRHYDRO_EINVAL, "bad max_patches / nslots");
+  if (bytes < need) return fail(h, AMRHYDRO_ENOMEM, "pool smaller than amrhydro_pool_bytes()");
+  if ((uintptr_t)dev_pool % 256) return fail(h, AMRHYDRO_EINVAL, "pool must be 256-byte aligned");
+  h->pool = dev_pool; h->pool_bytes = bytes; h->maxp = max_patches; h->nslots = nslots;
+  h->stream = (cudaStream_t)stream;
+  h->bound = true;
+  CUDA_TRY(h, cudaMemsetAsync(dev_pool, 0, need, h->stream));
+  return 0;
+}
+
+int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
+  if (int r = check_ready(h, false)) return r;
+  if (!tbl || !bc || np <= 0 || nlev <= 0 || !(dx0 > 0)) return fail(h, AMRHYDRO_EINVAL, "bad hierarchy arguments");
+  if (np > h->maxp) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
+  std::vector<int> first(nlev, -1), count(nlev, 0), child(size_t(np) * 8, -1), octant(np, 0);
+  for (int p = 0; p < np; ++p) {
+    const auto &d = tbl[p];
+    if (d.level < 0 || d.level >= nlev) return fail(h, AMRHYDRO_EINVAL, "patch level out of range");
+    if (p > 0 && d.level < tbl[p - 1].level) return fail(h, AMRHYDRO_EINVAL, "patches must be sorted by level");
+    if (first[d.level] < 0) first[d.level] = p;
+    ++count[d.level];
+    for (int r = 0; r < 27; ++r)
+      if (r != 13 && (d.nbr[r] >= np || d.nbr[r] < -2 || (d.nbr[r] >= 0 && tbl[d.nbr[r]].level != d.level)))
+        return fail(h, AMRHYDRO_EINVAL, "bad neighbour entry");
+    if (d.level == 0) {
+      for (int r = 0; r < 27; ++r)
+        if (r != 13 && d.nbr[r] == -1) return fail(h, AMRHYDRO_EINVAL, "level 0 cannot have coarse-fine faces");
+      continue;
+    }
+    int Q = d.parent;
+    if (Q < 0 || Q >= np || tbl[Q].level != d.level - 1) return fail(h, AMRHYDRO_EINVAL, "bad parent");
+    int o = 0;
+    for (int a = 0; a < 3; ++a) {
+      int rel = d.origin[a] - 2 * tbl[Q].origin[a];
+      if (rel != 0 && rel != NI) return fail(h, AMRHYDRO_EINVAL, "patch is not an octant of its parent");
+      if (rel == NI) o |= 1 << a;
+    }
+    octant[p] = o;
+    if (child[size_t(Q) * 8 + o] >= 0) return fail(h, AMRHYDRO_EINVAL, "two patches refine the same octant");
+    child[size_t(Q) * 8 + o] = p;
+    for (int f = 0; f < 6; ++f) {              // proper nesting: the uncovered coarse cell must exist
+      if (d.nbr[face_region(f)] != -1) continue;
+      int a = f >> 1, hi = f & 1, bit = (o >> a) & 1;
+      if (((hi && bit == 1) || (!hi && bit == 0)) && tbl[Q].nbr[face_region(f)] < 0)
+        return fail(h, AMRHYDRO_EINVAL, "improper nesting: fine face on a coarse-fine/physical parent face");
+    }
+  }
+  for (int l = 0; l < nlev; ++l)
+    if (count[l] == 0) return fail(h, AMRHYDRO_EINVAL, "empty level");
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  free_hierarchy(h);
+  h->tbl.assign(tbl, tbl + np);
+  h->child = child; h->octant = octant; h->lev_first = first; h->lev_count = count;
+  h->nlev = nlev; h->dx0 = dx0;
+  for (int i = 0; i < 6; ++i) h->bc[i] = bc[i];
+  CUDA_TRY(h, cudaMalloc(&h->d_desc, size_t(np) * sizeof(Desc)));
+  CUDA_TRY(h, cudaMalloc(&h->d_child, size_t(np) * 8 * sizeof(int)));
+  CUDA_TRY(h, cudaMalloc(&h->d_octant, size_t(np) * sizeof(int)));
+  CUDA_TRY(h, cudaMemcpy(h->d_desc, tbl, size_t(np) * sizeof(Desc), cudaMemcpyHostToDevice));
+  CUDA_TRY(h, cudaMemcpy(h->d_child, child.data(), size_t(np) * 8 * sizeof(int), cudaMemcpyHostToDevice));
+  CUDA_TRY(h, cudaMemcpy(h->d_octant, octant.data(), size_t(np) * sizeof(int), cudaMemcpyHostToDevice));
+  if (nlev > 1) {
+    size_t rb = size_t(np) * 6 * h->nv * 64 * elem(h);
+    CUDA_TRY(h, cudaMalloc(&h->d_Rf, rb));
+    CUDA_TRY(h, cudaMalloc(&h->d_Rc, rb));
+    CUDA_TRY(h, cudaMemset(h->d_Rf, 0, rb));
+    CUDA_TRY(h, cudaMemset(h->d_Rc, 0, rb));
+    size_t mx = *std::max_element(count.begin(), count.end());
+    CUDA_TRY(h, cudaMalloc(&h->d_bflux, mx * 9 * h->nv * 256 * elem(h)));
+    h->bflux_patches = mx;
+  }
+  h->np = np;
+  return 0;
+}
+
+int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *host) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!host || first < 0 || count < 0 || first + count > h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  const size_t per = size_t(h->nv) * 4096 * elem(h);
+  const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
+  if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
+  for (int done = 0; done < count; done += chunk) {
+    int n = std::min(chunk, count - done);
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_stage, (const char *)host + size_t(done) * per, size_t(n) * per,
+                                cudaMemcpyHostToDevice, h->stream));
+    int r = dispatch(h, [&](auto t, auto nv) {
+      using T = decltype(t);
+      k_pack<T><<<dim3(n, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, first + done, (const T *)h->d_stage);
+      LAUNCH_CHECK(h);
+      (void)nv;
+      return 0;
+    });
+    if (r) return r;
+  }
+  return 0;
+}
+
+int amrhydro_download(amrhydro_t *h, int slot, int first, int count, void *host) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!host || first < 0 || count < 0 || first + count > h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  const size_t per = size_t(h->nv) * 4096 * elem(h);
+  const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
+  if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
+  for (int done = 0; done < count; done += chunk) {
+    int n = std::min(chunk, count - done);
+    int r = dispatch(h, [&](auto t, auto nv) {
+      using T = decltype(t);
+      k_unpack<T><<<dim3(n, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, first + done, (T *)h->d_stage);
+      LAUNCH_CHECK(h);
+      (void)nv;
+      return 0;
+    });
+    if (r) return r;
+    CUDA_TRY(h, cudaMemcpyAsync((char *)host + size_t(done) * per, h->d_stage, size_t(n) * per,
+                                cudaMemcpyDeviceToHost, h->stream));
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int amrhydro_download_padded(amrhydro_t *h, int slot, int patch, double *out) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!out || patch < 0 || patch >= h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch");
+  size_t bytes = size_t(h->nv) * NP * NP * NP * sizeof(double);
+  if (int r = ensure_stage(h, bytes)) return r;
+  int r = dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    k_unpack_padded<T><<<64, 256, 0, h->stream>>>(make_pool<T>(h), slot, patch, (double *)h->d_stage);
+    LAUNCH_CHECK(h);
+    (void)nv;
+    return 0;
+  });
+  if (r) return r;
+  CUDA_TRY(h, cudaMemcpyAsync(out, h->d_stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int amrhydro_download_registers(amrhydro_t *h, int patch, double *rf, double *rc) {
+  if (int r = check_ready(h)) return r;
+  if (!rf || !rc || patch < 0 || patch >= h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch");
+  size_t n = size_t(6) * h->nv * 64;
+  if (!h->d_Rf) { std::fill(rf, rf + n, 0.0); std::fill(rc, rc + n, 0.0); return 0; }
+  std::vector<char> a(n * elem(h)), b(n * elem(h));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  CUDA_TRY(h, cudaMemcpy(a.data(), (char *)h->d_Rf + size_t(patch) * n * elem(h), n * elem(h), cudaMemcpyDeviceToHost));
+  CUDA_TRY(h, cudaMemcpy(b.data(), (char *)h->d_Rc + size_t(patch) * n * elem(h), n * elem(h), cudaMemcpyDeviceToHost));
+  for (size_t i = 0; i < n; ++i) {
+    rf[i] = h->bits == 64 ? ((double *)a.data())[i] : double(((float *)a.data())[i]);
+    rc[i] = h->bits == 64 ? ((double *)b.data())[i] : double(((float *)b.data())[i]);
+  }
+  return 0;
+}
+
+// enqueue the max-speed reduction of one level into d_scalars[0] (not reset here)
+static int enqueue_cfl(amrhydro_t *h, int level, int slot) {
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    k_cfl<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level],
+                                                              make_params<T>(h), h->d_scalars, h->d_scalars + 1);
+    LAUNCH_CHECK(h);
+    return 0;
+  });
+}
+static int read_smax(amrhydro_t *h, double *smax) {
+  unsigned long long bits = 0;
+  CUDA_TRY(h, cudaMemcpyAsync(&bits, h->d_scalars, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  double s;
+  std::memcpy(&s, &bits, sizeof(s));
+  *smax = s;
+  if (!(s > 0.0) || !std::isfinite(s)) return fail(h, AMRHYDRO_ENONFINITE, "max signal speed is zero or not finite");
+  return 0;
+}
+
+int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_out, double *smax_out) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!dt_out) return fail(h, AMRHYDRO_EINVAL, "dt_out is null");
+  CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, sizeof(unsigned long long), h->stream));
+  if (int r = enqueue_cfl(h, level, slot)) return r;
+  double s = 0;
+  int r = read_smax(h, &s);
+  if (smax_out) *smax_out = s;
+  if (r) return r;
+  *dt_out = cfl * (h->dx0 / double(1 << level)) / s;
+  return 0;
+}
+
+int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (level > 0) {
+    if (int r = check_slot(h, pold)) return r;
+    if (int r = check_slot(h, pnew)) return r;
+  } else {
+    pold = pnew = slot;
+  }
+  // direct-halo mode: sibling copies are only needed where someone prolongates from this level
+  const int skip = (h->halo == 1 && level + 1 >= h->nlev) ? 1 : 0;
+  if (skip && h->nlev == 1) {
+    bool phys = false;
+    for (int f = 0; f < 6; ++f) phys |= (h->bc[f] == AMRHYDRO_BC_OUTFLOW);
+    if (!phys) return 0;   // periodic single level: nothing to materialise
+  }
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    k_fill_ghosts<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(
+        make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->bc[0], h->bc[1],
+        h->bc[2], h->bc[3], h->bc[4], h->bc[5], skip);
+    LAUNCH_CHECK(h);
+    return 0;
+  });
+}
+
+int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, double a, double b, double dt, double w) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (check_slot(h, sin) || check_slot(h, sbase) || check_slot(h, sout)) return AMRHYDRO_EINVAL;
+  if (sin == sout) return fail(h, AMRHYDRO_EINVAL, "slot_out must differ from slot_in (halo hazard)");
+  const bool regs = (w != 0.0) && h->nlev > 1;
+  const double hx = h->dx0 / double(1 << level);
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    const int n = h->lev_count[level], first = h->lev_first[level];
+    T *bflux = regs ? (T *)h->d_bflux : nullptr;
+    if (h->kernel == 0) {
+      k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
+                                                                T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
+      LAUNCH_CHECK(h);
+    } else {
+      int r = launch_rk_stage_tile<T, NV>(make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_tile: ") + cudaGetErrorString((cudaError_t)r));
+      LAUNCH_CHECK(h);
+    }
+    if (regs) {
+      k_flux_registers<T, NV><<<dim3(n, 54), 64, 0, h->stream>>>(first, level, h->d_desc, h->d_child, bflux,
+                                                                  (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt));
+      LAUNCH_CHECK(h);
+    }
+    return 0;
+  });
+}
+
+int amrhydro_restrict(amrhydro_t *h, int flev, int fslot, int cslot) {
+  if (int r = check_ready(h)) return r;
+  if (flev < 1 || flev >= h->nlev) return fail(h, AMRHYDRO_EINVAL, "fine_level out of range");
+  if (check_slot(h, fslot) || check_slot(h, cslot)) return AMRHYDRO_EINVAL;
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    k_restrict<T, NV><<<h->lev_count[flev], 256, 0, h->stream>>>(make_pool<T>(h), fslot, cslot, h->lev_first[flev],
+                                                                  h->d_desc, h->d_octant);
+    LAUNCH_CHECK(h);
+    return 0;
+  });
+}
+
+int amrhydro_reflux(amrhydro_t *h, int clev, int slot) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, clev)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (clev + 1 >= h->nlev) return 0;
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    for (int f = 0; f < 6; ++f) {
+      k_reflux<T, NV><<<h->lev_count[clev + 1], 64, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[clev + 1], f,
+                                                                     h->d_desc, h->d_octant, (T *)h->d_Rf, (T *)h->d_Rc,
+                                                                     T(h->dx0 / double(1 << clev)));
+      LAUNCH_CHECK(h);
+    }
+    return 0;
+  });
+}
+
+int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (check_slot(h, src) || check_slot(h, dst)) return AMRHYDRO_EINVAL;
+  if (src == dst) return 0;
+  const size_t per = size_t(h->nv) * vs(h) * elem(h);
+  char *base = (char *)h->pool;
+  CUDA_TRY(h, cudaMemcpyAsync(base + (size_t(dst) * h->maxp + h->lev_first[level]) * per,
+                              base + (size_t(src) * h->maxp + h->lev_first[level]) * per,
+                              size_t(h->lev_count[level]) * per, cudaMemcpyDeviceToDevice, h->stream));
+  return 0;
+}
+
+// S9 recursion; a1/a2 = time-interpolation weights of the parent data for the two ghost fills (S7)
+static int advance_level(amrhydro_t *h, int lev, double dt, double a1, double a2) {
+  const bool kids = lev + 1 < h->nlev;
+  const double w = h->nlev > 1 ? 0.5 : 0.0;
+  int r;
+  if ((r = amrhydro_fill_ghosts(h, lev, 0, 2, 0, a1))) return r;
+  if (kids && (r = amrhydro_copy_slot(h, lev, 0, 2))) return r;
+  if ((r = amrhydro_rk_stage(h, lev, 0, 0, 1, 0.0, 1.0, dt, w))) return r;      // U1 = Un + dt L(Un)
+  if ((r = amrhydro_fill_ghosts(h, lev, 1, 2, 0, a2))) return r;
+  if ((r = amrhydro_rk_stage(h, lev, 1, 0, 0, 0.5, 0.5, dt, w))) return r;      // Un+1 = (Un + U1 + dt L(U1))/2
+  if (kids) {
+    if ((r = amrhydro_fill_ghosts(h, lev, 0, 2, 0, a2))) return r;
+    if ((r = advance_level(h, lev + 1, 0.5 * dt, 0.0, 0.5))) return r;
+    if ((r = advance_level(h, lev + 1, 0.5 * dt, 0.5, 1.0))) return r;
+    if ((r = amrhydro_restrict(h, lev + 1, 0, 0))) return r;
+    if ((r = amrhydro_reflux(h, lev, 0))) return r;
+  }
+  return 0;
+}
+
+int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out) {
+  if (int r = check_ready(h)) return r;
+  if (h->nslots < (h->nlev > 1 ? 3 : 2)) return fail(h, AMRHYDRO_ESTATE, "advance needs 2 slots (3 with refinement)");
+  double dt = dt_fixed;
+  if (!(dt > 0.0)) {
+    CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, sizeof(unsigned long long), h->stream));
+    for (int l = 0; l < h->nlev; ++l)
+      if (int r = enqueue_cfl(h, l, 0)) return r;
+    double s = 0;
+    if (int r = read_smax(h, &s)) return r;
+    dt = cfl * h->dx0 / s;                                  // S4: dt_l = dt0 / 2^l
+  }
+  if (dt_out) *dt_out = dt;
+  return advance_level(h, 0, dt, 0.0, 0.0);
+}
+
+int amrhydro_advance_host(amrhydro_t *h, double cfl, double dt_fixed, int nsteps, const void *host_in, void *host_out,
+                          double *dt_last) {
+  if (int r = check_ready(h)) return r;
+  if (!host_in || !host_out || nsteps < 0) return fail(h, AMRHYDRO_EINVAL, "bad host buffers");
+  if (int r = amrhydro_upload(h, 0, 0, h->np, host_in)) return r;
+  for (int s = 0; s < nsteps; ++s)
+    if (int r = amrhydro_advance(h, cfl, dt_fixed, dt_last)) return r;
+  return amrhydro_download(h, 0, 0, h->np, host_out);
+}
+
+int amrhydro_sync(amrhydro_t *h) {
+  if (!h) return AMRHYDRO_EINVAL;
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+}  // extern "C"

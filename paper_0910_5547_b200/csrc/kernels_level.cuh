@@ -1,0 +1,277 @@
+// kernels_level.cuh -- level-wide kernels around the stage: CFL reduction (a1), ghost fill
+// (a2), restriction (a7), flux registers + refluxing (a8), host staging pack/unpack.
+// The paper leaves all of these on the CPU inside Enzo; readings S4-S10.
+#pragma once
+#include "layout.cuh"
+#include "physics.cuh"
+
+namespace amr {
+
+// ------------------------------------------------------------------ staging <-> pool
+// staging: [count][var][16][16][16] (host interior layout).  One block per (patch, var).
+template <typename T>
+__global__ void __launch_bounds__(256) k_pack(Pool<T> pool, int slot, int first, const T *__restrict__ stage) {
+  const int p = blockIdx.x, v = blockIdx.y;
+  T *dst = pool.patch(slot, first + p) + size_t(v) * Layout<T>::VS;
+  const T *src = stage + (size_t(p) * pool.nv + v) * (NI * NI * NI);
+  for (int c = threadIdx.x; c < NI * NI * NI; c += 256) {
+    int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
+    dst[cell<T>(k + NG, j + NG, i + NG)] = src[c];
+  }
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_unpack(Pool<T> pool, int slot, int first, T *__restrict__ stage) {
+  const int p = blockIdx.x, v = blockIdx.y;
+  const T *src = pool.patch(slot, first + p) + size_t(v) * Layout<T>::VS;
+  T *dst = stage + (size_t(p) * pool.nv + v) * (NI * NI * NI);
+  for (int c = threadIdx.x; c < NI * NI * NI; c += 256) {
+    int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
+    dst[c] = src[cell<T>(k + NG, j + NG, i + NG)];
+  }
+}
+// padded box of one patch as doubles [var][20][20][20] (tests)
+template <typename T>
+__global__ void k_unpack_padded(Pool<T> pool, int slot, int p, double *__restrict__ out) {
+  const T *src = pool.patch(slot, p);
+  const int n = pool.nv * NP * NP * NP;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n; c += gridDim.x * blockDim.x) {
+    int v = c / (NP * NP * NP), r = c % (NP * NP * NP);
+    int i = r % NP, j = (r / NP) % NP, k = r / (NP * NP);
+    out[c] = double(src[size_t(v) * Layout<T>::VS + cell<T>(k, j, i)]);
+  }
+}
+
+// ------------------------------------------------------------------ a1: CFL reduction (S4)
+// One block per patch; thread (j,i) walks k.  Block max by warp shuffles, then one atomicMax
+// on the bit pattern of a non-negative double (monotone as an unsigned integer).
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_cfl(Pool<T> pool, int slot, int first, Params<T> P,
+                                             unsigned long long *__restrict__ smax_bits,
+                                             unsigned long long *__restrict__ floor_hits) {
+  const T *Ub = pool.patch(slot, first + blockIdx.x);
+  const int i = threadIdx.x & 15, j = threadIdx.x >> 4;
+  T best = T(0);
+  int hits = 0;
+  bool bad = false;
+#pragma unroll 4
+  for (int k = 0; k < NI; ++k) {
+    T U[NV], W[NV];
+    const int c = cell<T>(k + NG, j + NG, i + NG);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) U[v] = Ub[size_t(v) * Layout<T>::VS + c];
+    cons_to_prim<T, NV>(U, W, P, hits);
+    T s = max_signal_speed<T, NV>(W, P);
+    bad |= !(s == s);
+    best = tmax(best, s);
+  }
+  double b = bad ? __longlong_as_double(0x7ff0000000000000LL) : double(best);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) b = fmax(b, __shfl_xor_sync(0xffffffffu, b, o));
+  __shared__ double wmax[8];
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = b;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    b = threadIdx.x < 8 ? wmax[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) b = fmax(b, __shfl_xor_sync(0xffffffffu, b, o));
+    if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(b));
+  }
+  if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
+}
+
+// ------------------------------------------------------------------ a2: ghost fill (S5-S7)
+template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
+  if (a > T(0) && b > T(0)) return tmin(a, b);
+  if (a < T(0) && b < T(0)) return tmax(a, b);
+  return T(0);
+}
+
+// One block per patch.  Phase 1: every ghost cell whose 16^3 neighbour block is a sibling is
+// copied from that sibling's interior; where it is a coarse-fine boundary it is prolongated
+// from the parent's padded box, conservative limited-linear (S6) in time-interpolated parent
+// data (S7).  Phase 2: zero-gradient outflow, x then y then z over the full padded extent.
+// skip_siblings: face/edge/corner copies are skipped (rk_stage reads siblings directly).
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
+                                                     int first, const Desc *__restrict__ desc,
+                                                     int bc0, int bc1, int bc2, int bc3, int bc4, int bc5,
+                                                     int skip_siblings) {
+  const int p = first + blockIdx.x;
+  const Desc &D = desc[p];
+  T *U = pool.patch(slot, p);
+  __shared__ int s_nbr[27];
+  __shared__ int s_org[3], s_porg[3];
+  if (threadIdx.x < 27) s_nbr[threadIdx.x] = D.nbr[threadIdx.x];
+  if (threadIdx.x < 3) {
+    s_org[threadIdx.x] = D.origin[threadIdx.x];
+    s_porg[threadIdx.x] = D.parent >= 0 ? desc[D.parent].origin[threadIdx.x] : 0;
+  }
+  __syncthreads();
+  const int Q = D.parent;
+  const T *Co = Q >= 0 ? pool.patch(pold, Q) : nullptr;
+  const T *Cn = Q >= 0 ? pool.patch(pnew, Q) : nullptr;
+  for (int c = threadIdx.x; c < NP * NP * NP; c += 256) {
+    const int i = c % NP, j = (c / NP) % NP, k = c / (NP * NP);
+    const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0);
+    const int oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
+    const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
+    const int r = (oz + 1) * 9 + (oy + 1) * 3 + (ox + 1);
+    if (r == 13) continue;
+    const int nb = s_nbr[r];
+    const int me = cell<T>(k, j, i);
+    if (nb >= 0) {
+      if (skip_siblings) continue;
+      const T *S = pool.patch(slot, nb);
+      const int sc = cell<T>(k - oz * NI, j - oy * NI, i - ox * NI);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + me] = S[size_t(v) * Layout<T>::VS + sc];
+    } else if (nb == -1 && Q >= 0) {
+      const int pad[3] = {i, j, k};
+      int pc[3];
+      T s[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const int g = s_org[d] + pad[d] - NG;        // fine global index (>= -2)
+        const int gc = (g + 64) / 2 - 32;            // floor(g/2) for g >= -64
+        s[d] = (g - 2 * gc == 0) ? T(-0.25) : T(0.25);
+        pc[d] = gc - s_porg[d] + NG;
+      }
+      const int c0 = cell<T>(pc[2], pc[1], pc[0]);
+      const int st[3] = {1, Layout<T>::PX, Layout<T>::PLANE};
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const T *o = Co + size_t(v) * Layout<T>::VS, *n = Cn + size_t(v) * Layout<T>::VS;
+        const T uc = (T(1) - alpha) * o[c0] + alpha * n[c0];
+        T val = uc;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+          const T up = (T(1) - alpha) * o[c0 + st[d]] + alpha * n[c0 + st[d]];
+          const T um = (T(1) - alpha) * o[c0 - st[d]] + alpha * n[c0 - st[d]];
+          val = val + s[d] * minmod2(up - uc, uc - um);
+        }
+        U[size_t(v) * Layout<T>::VS + me] = val;
+      }
+    }
+  }
+  const int bc[6] = {bc0, bc1, bc2, bc3, bc4, bc5};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    bool any = false;
+    for (int side = 0; side < 2; ++side) any |= (s_nbr[face_region(2 * d + side)] == -2 && bc[2 * d + side] == 1);
+    if (!any) continue;                            // block-uniform
+    __syncthreads();
+    for (int side = 0; side < 2; ++side) {
+      if (!(s_nbr[face_region(2 * d + side)] == -2 && bc[2 * d + side] == 1)) continue;
+      const int src = side == 0 ? NG : NG + NI - 1;
+      for (int t = threadIdx.x; t < NG * NP * NP; t += 256) {
+        const int g = t / (NP * NP), a = (t / NP) % NP, b = t % NP;
+        const int dst = side == 0 ? g : NG + NI + g;
+        int cs, cd;
+        if (d == 0) { cs = cell<T>(a, b, src); cd = cell<T>(a, b, dst); }
+        else if (d == 1) { cs = cell<T>(a, src, b); cd = cell<T>(a, dst, b); }
+        else { cs = cell<T>(src, a, b); cd = cell<T>(dst, a, b); }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + cd] = U[size_t(v) * Layout<T>::VS + cs];
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ a7: restriction (S8)
+// One block per fine patch; each thread produces coarse cells (pairwise tree sum, so that a
+// uniform state is restricted bitwise).
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_restrict(Pool<T> pool, int fslot, int cslot, int first,
+                                                  const Desc *__restrict__ desc, const int *__restrict__ octant) {
+  const int p = first + blockIdx.x;
+  const int Q = desc[p].parent, o = octant[p];
+  const int ocx = o & 1, ocy = (o >> 1) & 1, ocz = (o >> 2) & 1;
+  const T *Uf = pool.patch(fslot, p);
+  T *Uc = pool.patch(cslot, Q);
+  for (int t = threadIdx.x; t < 512 * NV; t += 256) {
+    const int v = t / 512, c = t % 512;
+    const int ci = c & 7, cj = (c >> 3) & 7, ck = c >> 6;
+    const T *f = Uf + size_t(v) * Layout<T>::VS;
+    auto F = [&](int dk, int dj, int di) { return f[cell<T>(NG + 2 * ck + dk, NG + 2 * cj + dj, NG + 2 * ci + di)]; };
+    const T s = ((F(0, 0, 0) + F(0, 0, 1)) + (F(0, 1, 0) + F(0, 1, 1))) +
+                ((F(1, 0, 0) + F(1, 0, 1)) + (F(1, 1, 0) + F(1, 1, 1)));
+    Uc[size_t(v) * Layout<T>::VS + cell<T>(NG + 8 * ocz + ck, NG + 8 * ocy + cj, NG + 8 * ocx + ci)] = T(0.125) * s;
+  }
+}
+
+// ------------------------------------------------------------------ flux registers (S10)
+// rk_stage leaves the fluxes through the faces 0, 8 and 16 of every interior line in
+// bflux[(patch_local*9 + d*3 + s)*NV + v][t2*16 + t1]  (s = face/8).  This kernel turns them
+// into register increments in a fixed order: task < 6 = fine side of this patch's face;
+// task >= 6 = coarse side under child (task-6)/6, face (task-6)%6.
+template <typename T, int NV>
+__global__ void __launch_bounds__(64) k_flux_registers(int first, int level, const Desc *__restrict__ desc,
+                                                       const int *__restrict__ child, const T *__restrict__ bflux,
+                                                       T *__restrict__ Rf, T *__restrict__ Rc, T wdt) {
+  const int pl = blockIdx.x, p = first + pl, task = blockIdx.y;
+  const int ca = threadIdx.x & 7, cb = threadIdx.x >> 3;
+  if (task < 6) {
+    const int f = task;
+    if (level == 0 || desc[p].nbr[face_region(f)] != -1) return;
+    const int d = f >> 1, s = (f & 1) ? 2 : 0;
+    T *R = Rf + (size_t(p) * 6 + f) * NV * 64;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const T *F = bflux + ((size_t(pl) * 9 + d * 3 + s) * NV + v) * 256;
+      const T sum = (F[(2 * cb) * 16 + 2 * ca] + F[(2 * cb) * 16 + 2 * ca + 1]) +
+                    (F[(2 * cb + 1) * 16 + 2 * ca] + F[(2 * cb + 1) * 16 + 2 * ca + 1]);
+      R[v * 64 + cb * 8 + ca] += wdt * (T(0.25) * sum);
+    }
+  } else {
+    const int o = (task - 6) / 6, f = (task - 6) % 6;
+    const int ch = child[size_t(p) * 8 + o];
+    if (ch < 0 || desc[ch].nbr[face_region(f)] != -1) return;
+    const int oc[3] = {o & 1, (o >> 1) & 1, (o >> 2) & 1};
+    const int d = f >> 1, s = oc[d] + (f & 1);
+    const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;
+    T *R = Rc + (size_t(ch) * 6 + f) * NV * 64;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const T *F = bflux + ((size_t(pl) * 9 + d * 3 + s) * NV + v) * 256;
+      R[v * 64 + cb * 8 + ca] += wdt * F[(8 * oc[d2] + cb) * 16 + 8 * oc[d1] + ca];
+    }
+  }
+}
+
+// ------------------------------------------------------------------ a8: refluxing (S10)
+// Launched once per face f = 0..5 (fixed order: a coarse cell is touched by at most one
+// fine face per launch, so there are no races and the rounding order is deterministic).
+template <typename T, int NV>
+__global__ void __launch_bounds__(64) k_reflux(Pool<T> pool, int slot, int first_fine, int f,
+                                               const Desc *__restrict__ desc, const int *__restrict__ octant,
+                                               T *__restrict__ Rf, T *__restrict__ Rc, T hc) {
+  const int p = first_fine + blockIdx.x;
+  if (desc[p].nbr[face_region(f)] != -1) return;
+  const int Q = desc[p].parent, o = octant[p];
+  const int oc[3] = {o & 1, (o >> 1) & 1, (o >> 2) & 1};
+  const int d = f >> 1, hi = f & 1;
+  const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;
+  int cn = NG + 8 * oc[d] + (hi ? 8 : -1);
+  int tgt = Q;
+  if (cn < NG || cn >= NG + NI) {
+    tgt = desc[Q].nbr[face_region(f)];
+    if (tgt < 0) return;                        // improper nesting is rejected by set_hierarchy
+    cn += hi ? -NI : NI;
+  }
+  T *U = pool.patch(slot, tgt);
+  T *rf = Rf + (size_t(p) * 6 + f) * NV * 64, *rc = Rc + (size_t(p) * 6 + f) * NV * 64;
+  const int ca = threadIdx.x & 7, cb = threadIdx.x >> 3;
+  int pad[3];
+  pad[d] = cn; pad[d1] = NG + 8 * oc[d1] + ca; pad[d2] = NG + 8 * oc[d2] + cb;
+  const int c = cell<T>(pad[2], pad[1], pad[0]);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const int r = v * 64 + cb * 8 + ca;
+    const T corr = (rf[r] - rc[r]) / hc;
+    T *u = U + size_t(v) * Layout<T>::VS + c;
+    *u = hi ? (*u + corr) : (*u - corr);
+    rf[r] = T(0); rc[r] = T(0);
+  }
+}
+
+}  // namespace amr

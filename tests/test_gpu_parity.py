@@ -1,0 +1,274 @@
+"""GPU parity: every C-ABI call against the CPU oracle, element by element, on the same seeded
+inputs (norm S14; tolerances 1e-12 fp64, 1e-5 fp32 from BASELINE.json)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_0910_5547_b200 import workloads as wl  # noqa: E402
+from util import norm_err  # noqa: E402
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_0910_5547_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def make_pair(gpu, h, gamma, nv, dtype="f64", ncpu=8, **kw):
+    import oracle
+    g = gpu.AmrHydro(h, gamma, nv, dtype=dtype, **kw)
+    o = oracle.Oracle(h, gamma, nv, threads=ncpu, theta=kw.get("theta", 1.5))
+    return g, o
+
+
+def upload_both(g, o, U, dtype):
+    if dtype == "f32":
+        U = U.astype(np.float32).astype(np.float64)   # S15: both start from the fp32-rounded data
+    g.upload(0, U)
+    o.upload(0, U)
+    return U
+
+
+def rand_state(h, nv, seed, gamma=1.4):
+    rng = np.random.default_rng(seed)
+    n = len(h["level"])
+    shp = (n, 16, 16, 16)
+    rho = rng.uniform(0.5, 1.5, shp); p = rng.uniform(0.5, 1.5, shp)
+    v = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)]
+    B = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)] if nv == 8 else None
+    return np.moveaxis(wl.cons_from_prim(rho, p, v, gamma, B=B), 0, 1).copy()
+
+
+# ------------------------------------------------------------------ a1: CFL reduction
+@pytest.mark.parametrize("nv,dtype", [(5, "f64"), (8, "f64"), (5, "f32"), (8, "f32")])
+def test_cfl_dt_matches_oracle(gpu, nv, dtype):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 1.4, nv, dtype)
+    upload_both(g, o, rand_state(h, nv, 1), dtype)
+    tol = 1e-14 if dtype == "f64" else 2e-6
+    assert abs(g.max_speed(0) - o.max_speed(0)) <= tol * o.max_speed(0)
+    assert abs(g.cfl_dt(0, 0, 0.3) - o.cfl_dt(0, 0, 0.3)) <= tol * o.cfl_dt(0, 0, 0.3)
+
+
+def test_cfl_dt_reports_nonfinite(gpu):
+    h = wl.uniform_hierarchy(1, periodic=True)
+    g = gpu.AmrHydro(h, 1.4, 5)
+    U = rand_state(h, 5, 2)
+    U[0, 1, 3, 3, 3] = np.nan
+    g.upload(0, U)
+    with pytest.raises(gpu.AmrHydroError):
+        g.cfl_dt(0, 0, 0.3)
+
+
+# ------------------------------------------------------------------ a2: ghost fill
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_fill_ghosts_single_level_bit_exact(gpu, periodic, dtype):
+    h = wl.uniform_hierarchy(2, periodic=periodic)
+    g, o = make_pair(gpu, h, 1.4, 5, dtype)
+    upload_both(g, o, rand_state(h, 5, 3), dtype)
+    g.fill_ghosts(0, 0); o.fill_ghosts(0, 0)
+    P = o.download_padded(0)
+    for p in range(8):
+        assert np.array_equal(g.download_padded(0, p), P[p])
+
+
+def amr_hier(kind):
+    if kind == "centre":
+        return wl.build_hierarchy((2, 2, 2), [[(i, j, k) for i in (1, 2) for j in (1, 2) for k in (1, 2)]], (0,) * 6)
+    if kind == "slab":
+        return wl.build_hierarchy((2, 2, 2), [[(i, j, k) for i in (2, 3) for j in (1, 2) for k in range(4)]], (0,) * 6)
+    return wl.ball_hierarchy(2, 3, bc=(1,) * 6)
+
+
+@pytest.mark.parametrize("kind", ["centre", "slab", "ball"])
+@pytest.mark.parametrize("alpha", [0.0, 0.5])
+def test_fill_ghosts_prolongation_matches_oracle(gpu, kind, alpha):
+    h = amr_hier(kind)
+    g, o = make_pair(gpu, h, 1.4, 5)
+    Ua, Uc = rand_state(h, 5, 4), rand_state(h, 5, 5)
+    for x, slot in ((g, None), (o, None)):
+        x.upload(0, Ua); x.upload(2, Uc); x.upload(1, Ua * 0.5)
+    for lev in range(h["nlevels"]):
+        for x in (g, o):
+            x.fill_ghosts(lev, 0, 2, 0, 0.0)
+            x.fill_ghosts(lev, 2, 2, 0, 0.0)
+            x.fill_ghosts(lev, 1, 2, 0, alpha)
+    P = o.download_padded(1)
+    worst = 0.0
+    for p in range(len(h["level"])):
+        G = g.download_padded(1, p)
+        # the oracle leaves untouched cells at 0; compare everything the fill defines
+        worst = max(worst, np.abs(G - P[p]).max())
+    assert worst <= 4e-16 * 2.0, worst
+
+
+# ------------------------------------------------------------------ a3-a6: one stage
+@pytest.mark.parametrize("nv", [5, 8])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kernel,halo", [(0, 0), (1, 0), (1, 1)])
+def test_rk_stage_matches_oracle(gpu, nv, dtype, kernel, halo):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, nv, dtype, kernel=kernel, halo=halo)
+    upload_both(g, o, rand_state(h, nv, 6, 5.0 / 3.0), dtype)
+    dt = 0.3 * o.cfl_dt(0, 0, 1.0)
+    for x in (g, o):
+        x.fill_ghosts(0, 0)
+        x.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
+        x.fill_ghosts(0, 1)
+        x.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+    assert norm_err(g.download(1).astype(np.float64), o.download(1)).max() <= TOL[dtype]
+    assert norm_err(g.download(0).astype(np.float64), o.download(0)).max() <= TOL[dtype]
+
+
+@pytest.mark.parametrize("theta", [0.0, 1.0, 2.0])
+def test_rk_stage_theta_option(gpu, theta):
+    h = wl.uniform_hierarchy(1, periodic=True)
+    g, o = make_pair(gpu, h, 1.4, 5, theta=theta)
+    upload_both(g, o, rand_state(h, 5, 7), "f64")
+    for x in (g, o):
+        x.fill_ghosts(0, 0)
+        x.rk_stage(0, 0, 0, 1, 0.0, 1.0, 1e-3)
+    assert norm_err(g.download(1), o.download(1)).max() <= 1e-13
+
+
+def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
+    h = wl.uniform_hierarchy(2, periodic=False)
+    U = rand_state(h, 5, 8)
+    res = []
+    for kernel, halo in ((0, 0), (1, 0), (1, 1)):
+        g = gpu.AmrHydro(h, 1.4, 5, kernel=kernel, halo=halo)
+        g.upload(0, U)
+        g.fill_ghosts(0, 0)
+        g.rk_stage(0, 0, 0, 1, 0.0, 1.0, 1e-3)
+        res.append(g.download(1))
+    assert norm_err(res[1], res[0]).max() <= 1e-14
+    assert np.array_equal(res[1], res[2])      # halo source does not change the arithmetic
+
+
+def test_uniform_state_bitwise_on_gpu(gpu):
+    h = wl.ball_hierarchy(2, 3, bc=(1,) * 6)
+    n = len(h["level"])
+    one = np.ones((n, 16, 16, 16))
+    U = np.moveaxis(wl.cons_from_prim(1.3 * one, 0.7 * one, (0.3 * one, -0.2 * one, 0.9 * one), 1.4), 0, 1).copy()
+    g = gpu.AmrHydro(h, 1.4, 5)
+    g.upload(0, U)
+    for _ in range(2):
+        g.advance(0.3)
+    assert np.array_equal(g.download(0), U)
+
+
+# ------------------------------------------------------------------ a7 / a8 and the registers
+@pytest.mark.parametrize("kind", ["centre", "slab"])
+def test_restrict_reflux_registers_match_oracle(gpu, kind):
+    h = amr_hier(kind)
+    g, o = make_pair(gpu, h, 1.4, 5)
+    U = rand_state(h, 5, 9)
+    g.upload(0, U); o.upload(0, U)
+    g.restrict(1); o.restrict(1)
+    assert norm_err(g.download(0), o.download(0)).max() <= 2e-16
+    dt = 1e-3
+    for x in (g, o):
+        for lev, d in ((0, dt), (1, dt / 2)):
+            x.fill_ghosts(lev, 0, 0, 0, 0.0)
+            x.rk_stage(lev, 0, 0, 1, 0.0, 1.0, d, 0.5)
+    nreg = 0
+    for p in wl.level_patches(h, 1):
+        rf, rc = g.download_registers(p)
+        of, oc = o.registers(p)
+        assert np.abs(rf - of).max() <= 1e-15 and np.abs(rc - oc).max() <= 1e-15
+        nreg += int((of != 0).any()) + int((oc != 0).any())
+    assert nreg > 0
+    g.reflux(0, 1); o.reflux(0, 1)
+    assert norm_err(g.download(1), o.download(1)).max() <= 1e-13
+    rf, rc = g.download_registers(int(wl.level_patches(h, 1)[0]))
+    assert not rf.any() and not rc.any()
+
+
+# ------------------------------------------------------------------ whole-path parity runs (configs)
+def run_both(g, o, steps, cfl, same_dt=True):
+    for _ in range(steps):
+        dt = o.advance(cfl)
+        dg = g.advance(cfl, dt if same_dt else 0.0)
+        assert abs(dg - dt) <= 1e-6 * dt
+    return g.download(0).astype(np.float64), o.download(0)
+
+
+def test_config1_sod_20_steps_fp64(gpu):
+    h = wl.uniform_hierarchy(2, periodic=False)
+    g, o = make_pair(gpu, h, 1.4, 5)
+    upload_both(g, o, wl.split_global(h, wl.sod_global(32)), "f64")
+    G, O = run_both(g, o, 20, 0.4, same_dt=False)     # the GPU computes its own dt here
+    assert norm_err(G, O).max() <= 1e-12
+    assert g.get_counter(gpu.CNT_FLOOR_HITS) == 0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("halo", [0, 1])
+def test_config2_kelvin_helmholtz_reduced(gpu, dtype, halo):
+    h = wl.uniform_hierarchy(4, periodic=True)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 5, dtype, halo=halo)
+    upload_both(g, o, wl.split_global(h, wl.kelvin_helmholtz_global(64)), dtype)
+    G, O = run_both(g, o, 10, 0.3)
+    assert norm_err(G, O).max() <= TOL[dtype]
+
+
+def test_config3_sedov_amr_5_levels(gpu):
+    h = wl.ball_hierarchy(4, 5, bc=(1,) * 6)
+    g, o = make_pair(gpu, h, 1.4, 5)
+    U = wl.sedov_hierarchy_state(h)
+    upload_both(g, o, U, "f64")
+    G, O = run_both(g, o, 2, 0.3)
+    assert np.isfinite(G).all()
+    assert norm_err(G, O).max() <= 1e-12
+    # composite conservation on the GPU: level-0 sums (covered cells hold restricted data)
+    l0 = wl.level_patches(h, 0)
+    tot0 = U[l0].sum(axis=(0, 2, 3, 4)); tot1 = G[l0].sum(axis=(0, 2, 3, 4))
+    assert abs(tot1[0] - tot0[0]) <= 1e-13 * tot0[0]
+
+
+@pytest.mark.parametrize("halo", [0, 1])
+def test_config4_mhd_reduced(gpu, halo):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 8, halo=halo)
+    upload_both(g, o, wl.split_global(h, wl.mhd_turbulence_global(32)), "f64")
+    G, O = run_both(g, o, 10, 0.3)
+    assert norm_err(G, O).max() <= 1e-12
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config5_stress_reduced(gpu, dtype):
+    h = wl.uniform_hierarchy(4, periodic=True)
+    g, o = make_pair(gpu, h, 1.4, 5, dtype, halo=1)
+    upload_both(g, o, wl.split_global(h, wl.stress_global(64)), dtype)
+    G, O = run_both(g, o, 3, 0.3)
+    assert norm_err(G, O).max() <= TOL[dtype]
+
+
+def test_amr_mhd_two_level(gpu):
+    h = amr_hier("slab")
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 8)
+    upload_both(g, o, rand_state(h, 8, 12, 5.0 / 3.0), "f64")
+    for x in (g, o):
+        x.restrict(1)
+    G, O = run_both(g, o, 2, 0.3)
+    assert norm_err(G, O).max() <= 1e-12
+
+
+def test_advance_host_end_to_end(gpu):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 1.4, 5)
+    U = rand_state(h, 5, 13)
+    o.upload(0, U)
+    dt = 0.3 * o.cfl_dt(0, 0, 1.0)
+    o.advance(0.3, dt); o.advance(0.3, dt)
+    out = np.empty_like(U)
+    g.advance_host(0.3, dt, 2, U.ctypes.data, out.ctypes.data)
+    assert norm_err(out, o.download(0)).max() <= 1e-12
