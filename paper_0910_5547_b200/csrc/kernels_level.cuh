@@ -61,7 +61,8 @@ __global__ void __launch_bounds__(256) k_cfl(Pool<T> pool, int slot, int first, 
     for (int v = 0; v < NV; ++v) U[v] = Ub[size_t(v) * Layout<T>::VS + c];
     cons_to_prim<T, NV>(U, W, P, hits);
     T s = max_signal_speed<T, NV>(W, P);
-    bad |= !(s == s);
+    const T chk = ((W[2] + W[3]) + W[4]) + s;      // fmax drops NaNs: test the operands themselves
+    bad |= !(chk - chk == T(0));                   // NaN or inf anywhere
     best = tmax(best, s);
   }
   double b = bad ? __longlong_as_double(0x7ff0000000000000LL) : double(best);

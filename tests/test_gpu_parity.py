@@ -217,7 +217,7 @@ def test_config2_kelvin_helmholtz_reduced(gpu, dtype, halo):
     g, o = make_pair(gpu, h, 5.0 / 3.0, 5, dtype, halo=halo)
     upload_both(g, o, wl.split_global(h, wl.kelvin_helmholtz_global(64)), dtype)
     G, O = run_both(g, o, 10, 0.3)
-    assert norm_err(G, O).max() <= TOL[dtype]
+    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
 
 
 def test_config3_sedov_amr_5_levels(gpu):
@@ -249,7 +249,7 @@ def test_config5_stress_reduced(gpu, dtype):
     g, o = make_pair(gpu, h, 1.4, 5, dtype, halo=1)
     upload_both(g, o, wl.split_global(h, wl.stress_global(64)), dtype)
     G, O = run_both(g, o, 3, 0.3)
-    assert norm_err(G, O).max() <= TOL[dtype]
+    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
 
 
 def test_amr_mhd_two_level(gpu):
