@@ -17,6 +17,7 @@
 #include "physics.cuh"
 #include "rk_stage_ref.cuh"
 #include "rk_stage_tile.cuh"
+#include "rk_stage_march.cuh"
 
 using namespace amr;
 
@@ -26,7 +27,7 @@ struct amrhydro {
   double gamma = 1.4;
   int nv = 5, bits = 64;
   double theta = 1.5, rho_floor = 1e-30, e_floor = 1e-30;
-  int kernel = 1, halo = 0;
+  int kernel = 2, halo = 0;
   void *pool = nullptr;
   size_t pool_bytes = 0;
   int maxp = 0, nslots = 0;
@@ -45,6 +46,8 @@ struct amrhydro {
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
+  CUtensorMap tmap;            // TMA view of the pool (rk_stage_march)
+  bool have_tmap = false;
   std::string err;
 };
 
@@ -164,10 +167,13 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
       if (!(value >= 0.0 && value <= 2.0)) return fail(h, AMRHYDRO_EINVAL, "theta must lie in [0,2]");
       h->theta = value;
       return 0;
-    case AMRHYDRO_OPT_RHO_FLOOR: h->rho_floor = value; return 0;
-    case AMRHYDRO_OPT_EINT_FLOOR: h->e_floor = value; return 0;
+    case AMRHYDRO_OPT_RHO_FLOOR:
+    case AMRHYDRO_OPT_EINT_FLOOR:
+      if (!(value > 0.0) || !std::isfinite(value)) return fail(h, AMRHYDRO_EINVAL, "floors must be positive and finite");
+      (key == AMRHYDRO_OPT_RHO_FLOOR ? h->rho_floor : h->e_floor) = value;
+      return 0;
     case AMRHYDRO_OPT_KERNEL:
-      if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0 or 1");
+      if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0, 1 or 2");
       h->kernel = int(value);
       return 0;
     case AMRHYDRO_OPT_HALO:
@@ -210,6 +216,14 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   h->pool = dev_pool; h->pool_bytes = bytes; h->maxp = max_patches; h->nslots = nslots;
   h->stream = (cudaStream_t)stream;
   h->bound = true;
+  {
+    int r = dispatch(h, [&](auto t, auto nv) {
+      using T = decltype(t);
+      return make_tensor_map<T, decltype(nv)::value>(&h->tmap, dev_pool, size_t(max_patches), nslots);
+    });
+    h->have_tmap = (r == 0);
+    if (r) { h->bound = false; return fail(h, AMRHYDRO_ECUDA, "cuTensorMapEncodeTiled failed for the pool"); }
+  }
   CUDA_TRY(h, cudaMemsetAsync(dev_pool, 0, need, h->stream));
   return 0;
 }
@@ -441,6 +455,11 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
                                                                 T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
+      LAUNCH_CHECK(h);
+    } else if (h->kernel == 2) {
+      int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                           make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
     } else {
       int r = launch_rk_stage_tile<T, NV>(make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),

@@ -1,0 +1,573 @@
+// rk_stage_march.cuh -- the hot kernel: one method-of-lines stage of every 16^3 patch of a level
+// (steps a3-a6: PAPER.md:79 Eq. 7, :94-98 Eq. 8, :104-112 Eq. 9-11, :114-118 Eq. 12).
+//
+// B200 design (the paper's 1-D flattened sweeps with one global round trip per kernel,
+// PAPER.md:139-153 / :226-248, are prior art, not the blueprint).  ncu on the first versions of
+// this kernel showed the stage is bound by instruction issue, the FP64 pipe and the shared-memory
+// crossbar, not by HBM (profiles/README.md), so everything here is written for instruction count
+// and for keeping global-memory latency off the critical path:
+//  * one CTA per patch, 10 warps: 8 "interior" warps own the 16x16 (i,j) columns and march in z
+//    over the 20 padded planes; warp 8 owns the x-halo columns, warp 9 the y-halo rows.
+//    Fluxes, L(U) and primitives never touch HBM.
+//  * the 16x16xNV interior box of every plane is brought in by TMA (cp.async.bulk.tensor, one
+//    request per plane, 3-slot ring, mbarrier completion), issued two planes ahead by one
+//    elected thread: no load instructions, address arithmetic or prefetch registers in the
+//    interior warps, and the raw U of the cell being finished is still in the ring for the
+//    Runge-Kutta combination.  z-ghost planes come through the same ring (from this patch's ghost
+//    zones, or with AMRHYDRO_OPT_HALO=1 from the z-neighbour's interior).
+//  * each cell is converted to primitives once (one MUFU reciprocal + a third-order correction)
+//    and published in a double-buffered shared-memory plane for the x/y neighbours; the z stencil
+//    lives in registers; x/y exchange the cell-edge state q+ and the face fluxes through shared
+//    memory (two barriers per plane): each slope and each face flux is computed once.
+//  * the 1/2 of Eq. 12 and of the PLM half-slope are folded into constants (exact power-of-two
+//    scalings): the kernel carries G = 2F and sm = 4*(half slope).  Limiter without explicit
+//    |x| (the FP64 pipe would pay a DADD for each): compares and multiplies take |x| as an
+//    operand modifier, the sign is restored on the integer pipe.  Floors are tested on the high
+//    words (integer pipe) and applied in a rarely taken branch.
+#pragma once
+#include <cuda.h>
+
+#include "layout.cuh"
+#include "physics.cuh"
+
+namespace amr {
+namespace mk {
+
+// ---- fast reciprocal / square root (MUFU seed + one third-order step: error ~ seed^3)
+__device__ __forceinline__ double frcp(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));   // >= 20 good bits
+  double e = fma(-x, y, 1.0);
+  e = fma(e, e, e);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ float frcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// sqrt of a strictly positive, finite x
+__device__ __forceinline__ double fsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);              // (1 - x y^2)/2
+  r = r * fma(1.5, r, 1.0);                // (1-2r)^(-1/2) = 1 + r + 1.5 r^2 + O(r^3)
+  return fma(g, r, g);
+}
+__device__ __forceinline__ float fsqrt(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// x < fl for fl > 0 by integer order of the bit patterns (negative x and -0 compare below;
+// a positive NaN does not -- NaNs are reported by cfl_dt, not repaired here)
+__device__ __forceinline__ bool below(double x, double fl) { return __double_as_longlong(x) < __double_as_longlong(fl); }
+__device__ __forceinline__ bool below(float x, float fl) { return __float_as_int(x) < __float_as_int(fl); }
+__device__ __forceinline__ int hiw(double x) { return __double2hiint(x); }
+__device__ __forceinline__ int hiw(float x) { return __float_as_int(x); }
+// cheap necessary condition for "a or b is below fl": one integer min + one compare
+template <typename T> __device__ __forceinline__ bool maybe_below(T a, T b, T fl) { return min(hiw(a), hiw(b)) <= hiw(fl); }
+
+// sm = 4 * (1/2) minmod(theta dm, theta dp, c/2), c = qp - qm   (Eq. 9-11 with G1):
+// q-(cell) = q0 - sm/4, q+(cell) = q0 + sm/4.  theta2 = 2 theta.  Exactly the oracle's value when
+// c = qp - qm: min commutes with the monotone rounding of theta*x, all scalings are powers of two.
+template <typename T> __device__ __forceinline__ T slope4(T dm, T dp, T c, T theta2) {
+  const T m1 = tabs(dm) < tabs(dp) ? dm : dp;
+  const T t2 = theta2 * tabs(m1);
+  const T mr = t2 < tabs(c) ? t2 : c;
+  return same_sign(dm, dp) ? with_sign_of(mr, dm) : T(0);
+}
+
+// O1: conserved -> primitive W = (rho, e, vx, vy, vz, [Bx, By, Bz]);  PAPER.md:59, :298; floors S11
+template <typename T, int NV>
+__device__ __forceinline__ void prim(const T (&U)[NV], T (&W)[NV], const Params<T> &P, int &hits) {
+  T rho = U[0];
+  if (hiw(rho) <= hiw(P.rho_floor)) {
+    if (below(rho, P.rho_floor)) { rho = P.rho_floor; ++hits; }
+  }
+  const T ir = frcp(rho);
+  const T vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
+  T et = U[4];
+  if (NV == 8) {
+    et = fma(T(-0.5), fma(U[7 % NV], U[7 % NV], fma(U[6 % NV], U[6 % NV], U[5 % NV] * U[5 % NV])), et);
+    W[5 % NV] = U[5 % NV]; W[6 % NV] = U[6 % NV]; W[7 % NV] = U[7 % NV];
+  }
+  T e = fma(T(-0.5), fma(vz, vz, fma(vy, vy, vx * vx)), et * ir);
+  if (hiw(e) <= hiw(P.e_floor)) {
+    if (below(e, P.e_floor)) { e = P.e_floor; ++hits; }
+  }
+  W[0] = rho; W[1] = e; W[2] = vx; W[3] = vy; W[4] = vz;
+}
+
+template <typename T, int NV>
+__device__ __forceinline__ void floor_states2(T (&L)[NV], T (&R)[NV], T (&L2)[NV], T (&R2)[NV], const Params<T> &P, int &hits) {
+  const int hr = min(min(hiw(L[0]), hiw(R[0])), min(hiw(L2[0]), hiw(R2[0])));
+  const int he = min(min(hiw(L[1]), hiw(R[1])), min(hiw(L2[1]), hiw(R2[1])));
+  if ((hr <= hiw(P.rho_floor)) | (he <= hiw(P.e_floor))) {
+    if (below(L[0], P.rho_floor)) { L[0] = P.rho_floor; ++hits; }
+    if (below(L[1], P.e_floor)) { L[1] = P.e_floor; ++hits; }
+    if (below(R[0], P.rho_floor)) { R[0] = P.rho_floor; ++hits; }
+    if (below(R[1], P.e_floor)) { R[1] = P.e_floor; ++hits; }
+    if (below(L2[0], P.rho_floor)) { L2[0] = P.rho_floor; ++hits; }
+    if (below(L2[1], P.e_floor)) { L2[1] = P.e_floor; ++hits; }
+    if (below(R2[0], P.rho_floor)) { R2[0] = P.rho_floor; ++hits; }
+    if (below(R2[1], P.e_floor)) { R2[1] = P.e_floor; ++hits; }
+  }
+}
+template <typename T, int NV>
+__device__ __forceinline__ void floor_states(T (&L)[NV], T (&R)[NV], const Params<T> &P, int &hits) {
+  if (maybe_below(L[0], R[0], P.rho_floor) | maybe_below(L[1], R[1], P.e_floor)) {
+    if (below(L[0], P.rho_floor)) { L[0] = P.rho_floor; ++hits; }
+    if (below(L[1], P.e_floor)) { L[1] = P.e_floor; ++hits; }
+    if (below(R[0], P.rho_floor)) { R[0] = P.rho_floor; ++hits; }
+    if (below(R[1], P.e_floor)) { R[1] = P.e_floor; ++hits; }
+  }
+}
+
+// O3, Eq. 12 doubled: G = F(L) + F(R) - lambda0 (U(R) - U(L)),
+// lambda0 = max(|v_l| + c_l, |v_r| + c_r)  (= the max of Eq. 12 for single-valued c >= 0).
+template <typename T, int D>
+__device__ __forceinline__ void face_flux(const T (&L)[5], const T (&R)[5], const Params<T> &P, T (&G)[5]) {
+  const T rl = L[0], el = L[1], rr = R[0], er = R[1];
+  const T vdl = L[2 + D], vdr = R[2 + D];
+  const T rel = rl * el, rer = rr * er;
+  const T pl = P.gm1 * rel, pr = P.gm1 * rer;                                    // Eq. 6
+  const T ml = rl * vdl, mr = rr * vdr;
+  const T q2l = fma(L[4], L[4], fma(L[3], L[3], L[2] * L[2]));
+  const T q2r = fma(R[4], R[4], fma(R[3], R[3], R[2] * R[2]));
+  const T El = fma(T(0.5) * rl, q2l, rel), Er = fma(T(0.5) * rr, q2r, rer);      // rho (v^2/2 + e)
+  const T sl = tabs(vdl) + fsqrt(P.gg1 * el), sr = tabs(vdr) + fsqrt(P.gg1 * er);   // S2
+  const T lam = sl > sr ? sl : sr;
+  G[0] = fma(-lam, rr - rl, ml + mr);
+#pragma unroll
+  for (int t = 0; t < 3; ++t) {
+    T S, Dm;
+    if (t == D) { S = fma(mr, vdr, fma(ml, vdl, pl + pr)); Dm = mr - ml; }
+    else        { S = fma(mr, R[2 + t], ml * L[2 + t]);    Dm = fma(rr, R[2 + t], -(rl * L[2 + t])); }
+    G[1 + t] = fma(-lam, Dm, S);
+  }
+  G[4] = fma(-lam, Er - El, fma(Er + pr, vdr, (El + pl) * vdl));                 // rho (v^2/2 + h) v_d
+}
+
+// ideal MHD, Eq. 15 with G3 and psi == 0 (S3'); fast magnetosonic speed along D (S3)
+template <typename T, int D>
+__device__ __forceinline__ void mhd_state(const T (&W)[8], const Params<T> &P, T (&U)[8], T (&F)[8], T &speed) {
+  const T rho = W[0], e = W[1], vd = W[2 + D];
+  const T re = rho * e, p = P.gm1 * re, m = rho * vd;
+  const T q2 = fma(W[4], W[4], fma(W[3], W[3], W[2] * W[2]));
+  const T Bx = W[5], By = W[6], Bz = W[7], Bd = W[5 + D];
+  const T B2 = fma(Bz, Bz, fma(By, By, Bx * Bx));
+  const T Bv = fma(Bz, W[4], fma(By, W[3], Bx * W[2]));
+  const T hB2 = T(0.5) * B2, pt = p + hB2;
+  const T E = fma(T(0.5) * rho, q2, re) + hB2;
+  U[0] = rho; U[1] = rho * W[2]; U[2] = rho * W[3]; U[3] = rho * W[4]; U[4] = E; U[5] = Bx; U[6] = By; U[7] = Bz;
+  F[0] = m;
+  F[1] = fma(m, W[2], -(Bx * Bd)); F[2] = fma(m, W[3], -(By * Bd)); F[3] = fma(m, W[4], -(Bz * Bd));
+  F[1 + D] += pt;
+  F[4] = fma(E + pt, vd, -(Bd * Bv));
+  F[5] = fma(vd, Bx, -(Bd * W[2])); F[6] = fma(vd, By, -(Bd * W[3])); F[7] = fma(vd, Bz, -(Bd * W[4]));
+  F[5 + D] = T(0);
+  const T ir = frcp(rho);
+  const T a2 = P.gg1 * e, s = fma(B2, ir, a2), bd2 = Bd * Bd * ir;
+  const T disc = fma(s, s, T(-4) * a2 * bd2);
+  // disc >= 0 analytically; rounding can leave it tiny or negative when a^2 = b^2 = b_d^2
+  const T sq = disc > T(1e-30) * s * s ? fsqrt(disc) : T(0);
+  speed = tabs(vd) + fsqrt(T(0.5) * (s + sq));
+}
+template <typename T, int D>
+__device__ __forceinline__ void face_flux(const T (&L)[8], const T (&R)[8], const Params<T> &P, T (&G)[8]) {
+  T UL[8], UR[8], FL[8], FR[8], sl, sr;
+  mhd_state<T, D>(L, P, UL, FL, sl);
+  mhd_state<T, D>(R, P, UR, FR, sr);
+  const T lam = sl > sr ? sl : sr;
+#pragma unroll
+  for (int v = 0; v < 8; ++v) G[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
+}
+
+// ---- TMA / mbarrier (PTX ISA: cp.async.bulk.tensor, mbarrier)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+  unsigned ok;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int x, int y, int z, int q,
+                                            unsigned long long *bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+               ::"r"(smem_u32(dst)), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(q), "r"(smem_u32(bar)) : "memory");
+}
+
+template <typename T> struct Cfg;
+// shared-memory pitches: conflict-free for the row accesses of the interior warps (rows j, j+8
+// per warp) and for the column accesses of the x-halo warp
+template <> struct Cfg<double> { static constexpr int PW = 21, PQ = 17, PY = 16; };
+template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18; };
+
+constexpr int NSLOT = 4;      // TMA ring depth (raw conserved planes)
+
+template <typename T, int NV> struct Smem {
+  static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY;
+  static constexpr int RAWP = NV * NI * NI;        // one raw plane: [NV][16][16], dense TMA box
+  static constexpr int WV = NP * PW;               // one variable of one primitive plane [20][PW]
+  static constexpr int QXV = NI * PQ;              // [16][PQ]: slot s = q+ of cell s-1 / flux at face s
+  static constexpr int QYV = (NI + 1) * PY;        // [17][PY]
+  static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV, O_FX = O_QX + NV * QXV,
+                       O_QY = O_FX + NV * QXV, O_FY = O_QY + NV * QYV, O_END = O_FY + NV * QYV;
+  static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
+  static constexpr size_t BYTES = BAR_OFF + NSLOT * 8 + 128;   // + slack to align the ring to 128 B
+};
+
+#ifndef AMR_MINB64
+#define AMR_MINB64 1
+#endif
+#ifndef AMR_MINB32
+#define AMR_MINB32 3
+#endif
+constexpr int THREADS = 320;
+
+// One halo warp.  D = 0: lane = (row j, side): cells (-2,-1) or (16,17) of that row; D = 1: lane =
+// (column i, side): rows (-2,-1) or (16,17).  Converts its two cells of every interior plane,
+// publishes them next to the interior cells, computes the slope of the ghost cell adjacent to the
+// patch (q+ of cell -1 on the low side, q- of cell 16 on the high side) and, on the high side,
+// the flux through face 16.
+template <typename T, int NV, int D>
+__device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int lane, const Params<T> &P, T th2,
+                                          T *__restrict__ bflux, int pl, int &hits, bool producer,
+                                          const CUtensorMap *tmap, unsigned long long *bars, int q_mid, int q_lo,
+                                          int q_hi, int kz_lo, int kz_hi) {
+  using S = Smem<T, NV>;
+  constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV;
+  constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
+  constexpr int gst = D == 0 ? 1 : PX, rst = D == 0 ? 1 : PW;
+  constexpr int qv = D == 0 ? S::QXV : S::QYV;
+  const int t = lane & 15, hi = lane >> 4;
+  const T q4 = T(0.25);
+  // first of the two ghost cells (global, ring) and first of the three cells of the slope stencil
+  const T *g = (hi ? ghi : glo) + LEAD + (D == 0 ? (t + NG) * PX + (hi ? NG + NI : 0) : (hi ? NG + NI : 0) * PX + (t + NG));
+  T *W = sm + S::O_W;
+  T *r = W + (D == 0 ? (t + NG) * PW + (hi ? NG + NI : 0) : (hi ? NG + NI : 0) * PW + (t + NG));
+  const T *st3 = r + (hi ? -rst : 0);                       // cells (15,16,17) or (-2,-1,0)
+  T *Q = sm + (D == 0 ? S::O_QX : S::O_QY), *F = sm + (D == 0 ? S::O_FX : S::O_FY);
+  T *qlo = Q + (D == 0 ? t * PQ : t);                        // slot 0: q+ of cell -1
+  const T *qhi = Q + (D == 0 ? t * PQ + NI : NI * PY + t);   // slot 16: q+ of cell 15
+  T *fhi = F + (D == 0 ? t * PQ + NI : NI * PY + t);         // flux at face 16
+  T Ua[NV], Ub[NV];
+  auto load = [&](int pk) {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const T *s = g + size_t(v) * VS + pk * PLANE;
+      if (D == 0) {
+        if (sizeof(T) == 8) { const double2 x = *reinterpret_cast<const double2 *>(s); Ua[v] = T(x.x); Ub[v] = T(x.y); }
+        else                { const float2 x = *reinterpret_cast<const float2 *>(s);   Ua[v] = T(x.x); Ub[v] = T(x.y); }
+      } else {
+        Ua[v] = s[0]; Ub[v] = s[gst];
+      }
+    }
+  };
+  auto publish = [&](int pk) {
+    T W0[NV], W1[NV];
+    prim<T, NV>(Ua, W0, P, hits);
+    prim<T, NV>(Ub, W1, P, hits);
+    T *d = r + (pk & 1) * (NV * WV);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { d[v * WV] = W0[v]; d[v * WV + rst] = W1[v]; }
+  };
+  auto issue = [&](int pk) {                                  // TMA: interior box of padded plane pk
+    const int slot = pk % NSLOT;
+    const int q = pk < NG ? q_lo : (pk >= NG + NI ? q_hi : q_mid);
+    const int k = pk < NG ? pk + kz_lo : (pk >= NG + NI ? pk + kz_hi : pk);
+    mbar_expect_tx(&bars[slot], unsigned(S::RAWP * sizeof(T)));
+    tma_load_4d(sm + S::O_RAW + slot * S::RAWP, tmap, 0, NG, k, q, &bars[slot]);
+  };
+  if (producer) { issue(0); issue(1); issue(2); issue(3); }
+  load(NG);
+  publish(NG);
+  load(NG + 1);
+  __syncthreads();                                            // planes 0-2 converted by the interior warps
+  if (producer) issue(4);
+#pragma unroll 1
+  for (int c = NG; c < NG + NI; ++c) {
+    if (c + 1 < NG + NI) {
+      publish(c + 1);
+      if (c + 2 < NG + NI) load(c + 2);
+    }
+    const T *s3 = st3 + (c & 1) * (NV * WV);
+    T qm[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const T w0 = s3[v * WV], w1 = s3[v * WV + rst], w2 = s3[v * WV + 2 * rst];
+      const T s = slope4(w1 - w0, w2 - w1, w2 - w0, th2);
+      qm[v] = fma(-q4, s, w1);                                // q- of cell 16 (high side)
+      if (!hi) qlo[v * qv] = fma(q4, s, w1);                  // q+ of cell -1 (low side)
+    }
+    __syncthreads();
+    if (producer && c + 3 < NP) issue(c + 3);                 // slot of plane c-1 is free: cell c-1 is finished
+    if (hi) {
+      T WL[NV], G[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) WL[v] = qhi[v * qv];
+      floor_states<T, NV>(WL, qm, P, hits);
+      face_flux<T, D>(WL, qm, P, G);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) fhi[v * qv] = G[v];
+      if (bflux) {
+        T *B = bflux + ((size_t(pl) * 9 + 3 * D + 2) * NV) * 256 + (c - NG) * 16 + t;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace mk
+
+template <typename T, int NV, bool BASE>
+__global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : AMR_MINB32))
+k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
+                 T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
+                 const Desc *__restrict__ desc, int direct_halo) {
+  using S = mk::Smem<T, NV>;
+  constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
+  constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
+  extern __shared__ unsigned char smem_raw[];
+  // the TMA destination must be 128-byte aligned
+  T *sm = reinterpret_cast<T *>(smem_raw + ((128u - (mk::smem_u32(smem_raw) & 127u)) & 127u));
+  unsigned long long *bars = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(sm) + S::BAR_OFF);
+
+  const int pl = blockIdx.x, p = first + pl;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
+  const T th2 = T(2) * P.theta, q4 = T(0.25);
+  int hits = 0;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < mk::NSLOT; ++s) mk::mbar_init(&bars[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp < 8) {
+    // ------------------------------------------------------------------ interior columns
+    const int i = lane & 15, j = warp + 8 * (lane >> 4);
+    const int off = LEAD + (j + NG) * PX + (i + NG);            // in-plane offset of this column
+    const T *base = pool.patch(sbase, p) + off;
+    T *out = pool.patch(sout, p) + off;
+    const T *raw = sm + S::O_RAW + j * NI + i;                   // this column in ring slot 0, v = 0
+    T *wme = sm + S::O_W + (j + NG) * PW + (i + NG);             // this column in primitive plane 0, v = 0
+    T *qx = sm + S::O_QX + j * PQ + i, *fx = sm + S::O_FX + j * PQ + i;   // slot i: q+ of cell i-1 / flux at face i
+    T *qy = sm + S::O_QY + j * PY + i, *fy = sm + S::O_FY + j * PY + i;
+    T Wc[NV], dzm[NV], qpz[NV], acc[NV];
+    {
+      T U0[NV], U1[NV], U2[NV], W0[NV], W1[NV];
+      mk::mbar_wait(&bars[0], 0);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U0[v] = raw[v * (NI * NI)];
+      mk::mbar_wait(&bars[1], 0);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U1[v] = raw[RAWP + v * (NI * NI)];
+      mk::mbar_wait(&bars[2], 0);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U2[v] = raw[2 * RAWP + v * (NI * NI)];
+      mk::prim<T, NV>(U0, W0, P, hits);
+      mk::prim<T, NV>(U1, W1, P, hits);
+      mk::prim<T, NV>(U2, Wc, P, hits);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        wme[v * WV] = Wc[v];                                        // plane 2 -> primitive buffer 0
+        const T dm = W1[v] - W0[v];
+        dzm[v] = Wc[v] - W1[v];
+        const T s = mk::slope4(dm, dzm[v], Wc[v] - W0[v], th2);
+        qpz[v] = fma(q4, s, W1[v]);                                 // q+ of the ghost cell below plane 2
+        acc[v] = T(0);
+      }
+    }
+    __syncthreads();
+
+#pragma unroll 1
+    for (int c = NG; c <= NG + NI; ++c) {            // current cell = padded plane c (2..17); c = 18: last z face only
+      // 1. plane c+1: raw -> primitives, publish for the x/y neighbours
+      T Wn[NV];
+      {
+        const int slot = (c + 1) % mk::NSLOT;
+        mk::mbar_wait(&bars[slot], unsigned((c + 1) / mk::NSLOT) & 1u);
+        T Un[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Un[v] = raw[slot * RAWP + v * (NI * NI)];
+        mk::prim<T, NV>(Un, Wn, P, hits);
+      }
+      if (c + 1 < NG + NI) {
+        T *w = wme + ((c + 1) & 1) * (NV * WV);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) w[v * WV] = Wn[v];
+      }
+      T ub[NV];
+      if (BASE && c > NG) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) ub[v] = base[size_t(v) * VS + (c - 1) * PLANE];
+      }
+      // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
+      T Gz[NV];
+      {
+        T qm[NV], qp[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const T dp = Wn[v] - Wc[v];
+          const T s = mk::slope4(dzm[v], dp, dzm[v] + dp, th2);
+          qm[v] = fma(-q4, s, Wc[v]);
+          qp[v] = fma(q4, s, Wc[v]);
+          dzm[v] = dp;
+        }
+        mk::floor_states<T, NV>(qpz, qm, P, hits);
+        mk::face_flux<T, 2>(qpz, qm, P, Gz);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) qpz[v] = qp[v];
+      }
+      if (bflux && ((c - NG) & 7) == 0) {
+        T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG) >> 3)) * NV) * 256 + j * 16 + i;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gz[v];
+      }
+      if (c > NG) {
+        const T *ui = raw + ((c - 1) % mk::NSLOT) * RAWP;     // raw U of cell c-1 is still in the ring
+        T *o = out + (c - 1) * PLANE;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          T pre = b * ui[v * (NI * NI)];
+          if (BASE) pre = fma(a, ub[v], pre);
+          o[size_t(v) * VS] = fma(-kk, acc[v] + Gz[v], pre);        // Eq. 7-8
+        }
+      }
+      if (c < NG + NI) {
+        // 3. x/y phase 1: slopes of this cell along x and y, publish q+
+        const T *w = wme + (c & 1) * (NV * WV);
+        T qmx[NV], qmy[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const T wl = w[v * WV - 1], wr = w[v * WV + 1], wd = w[v * WV - PW], wu = w[v * WV + PW];
+          const T sx = mk::slope4(Wc[v] - wl, wr - Wc[v], wr - wl, th2);
+          const T sy = mk::slope4(Wc[v] - wd, wu - Wc[v], wu - wd, th2);
+          qmx[v] = fma(-q4, sx, Wc[v]);
+          qmy[v] = fma(-q4, sy, Wc[v]);
+          qx[v * QXV + 1] = fma(q4, sx, Wc[v]);
+          qy[v * QYV + PY] = fma(q4, sy, Wc[v]);
+        }
+        __syncthreads();
+        // 4. phase 2: fluxes through the low x and y faces of this cell
+        T Gx[NV], Gy[NV];
+        {
+          T WL[NV], WD[NV];
+#pragma unroll
+          for (int v = 0; v < NV; ++v) { WL[v] = qx[v * QXV]; WD[v] = qy[v * QYV]; }
+          mk::floor_states2<T, NV>(WL, qmx, WD, qmy, P, hits);
+          mk::face_flux<T, 0>(WL, qmx, P, Gx);
+          mk::face_flux<T, 1>(WD, qmy, P, Gy);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) { fx[v * QXV] = Gx[v]; fy[v * QYV] = Gy[v]; }
+        }
+        if (bflux) {
+          if ((i & 7) == 0) {
+            T *B = bflux + ((size_t(pl) * 9 + 0 + (i >> 3)) * NV) * 256 + (c - NG) * 16 + j;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx[v];
+          }
+          if ((j & 7) == 0) {
+            T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG) * 16 + i;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gy[v];
+          }
+        }
+        __syncthreads();
+        // 5. phase 3: flux differences in x and y; the low z face enters with its sign
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+          acc[v] = ((fx[v * QXV + 1] - Gx[v]) + (fy[v * QYV + PY] - Gy[v])) - Gz[v];
+      }
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Wc[v] = Wn[v];
+    }
+  } else {
+    // ------------------------------------------------------------------ halo warps (+ TMA producer)
+    const Desc &D = desc[p];
+    const T *self = pool.patch(sin, p);
+    const int f0 = warp == 8 ? 0 : 2;
+    const T *g[2];
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      const int nb = direct_halo ? D.nbr[face_region(f0 + s)] : -1;
+      const int st = warp == 8 ? 1 : PX;
+      g[s] = nb >= 0 ? pool.patch(sin, nb) + (s ? -NI * st : NI * st) : self;
+    }
+    const int nzl = direct_halo ? D.nbr[face_region(4)] : -1, nzh = direct_halo ? D.nbr[face_region(5)] : -1;
+    const int qbase = sin * pool.max_patches;
+    const int q_mid = (qbase + p) * NV, q_lo = (qbase + (nzl >= 0 ? nzl : p)) * NV, q_hi = (qbase + (nzh >= 0 ? nzh : p)) * NV;
+    const int kz_lo = nzl >= 0 ? NI : 0, kz_hi = nzh >= 0 ? -NI : 0;
+    if (warp == 8)
+      mk::halo_warp<T, NV, 0>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
+    else
+      mk::halo_warp<T, NV, 1>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
+  }
+  if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
+}
+
+// 4-D tensor map over the pool: (i, pj, pk, q) with q = (slot*max_patches + patch)*nv + var; the
+// origin is the first interior cell of a row, so that the global address is 32-byte aligned for
+// both element types.  Box = one interior plane of all variables of one patch.
+template <typename T, int NV>
+int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int nslots) {
+  typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn enc = nullptr;
+  if (!enc) {
+    void *fp = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess || !fp) return -1;
+    enc = (encode_fn)fp;
+  }
+  const cuuint64_t dims[4] = {cuuint64_t(NI), cuuint64_t(NP), cuuint64_t(NP), cuuint64_t(nslots) * max_patches * NV};
+  const cuuint64_t strides[3] = {cuuint64_t(Layout<T>::PX) * sizeof(T), cuuint64_t(Layout<T>::PLANE) * sizeof(T),
+                                 cuuint64_t(Layout<T>::VS) * sizeof(T)};
+  const cuuint32_t box[4] = {NI, NI, 1, NV};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  void *origin = (char *)pool_base + size_t(Layout<T>::LEAD + NG) * sizeof(T);
+  CUresult r = enc(tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, origin, dims,
+                   strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? 0 : -2;
+}
+
+// returns 0 or a cudaError_t
+template <typename T, int NV>
+int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
+                          T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
+                          cudaStream_t stream) {
+  static bool configured = false;
+  constexpr size_t bytes = mk::Smem<T, NV>::BYTES;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+    if (e != cudaSuccess) return int(e);
+    configured = true;
+  }
+  if (a != T(0))
+    k_rk_stage_march<T, NV, true><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
+                                                                     floor_hits, desc, direct_halo);
+  else
+    k_rk_stage_march<T, NV, false><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
+                                                                      floor_hits, desc, direct_halo);
+  return 0;
+}
+
+}  // namespace amr
