@@ -77,7 +77,7 @@ class AmrHydroError(RuntimeError):
 class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
-    def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=1, halo=0,
+    def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=2, halo=0,
                  rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():
