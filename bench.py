@@ -82,47 +82,57 @@ def make_workload(name, size, seed_shift=0):
 
 
 class ClockSampler:
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons sampled through NVML every ~5 ms by a thread while the
+    timed region runs (the recipe's nvidia-smi line starts too slowly for a region of ~0.1 s)."""
 
     def __init__(self, index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-        self.p = None
+        import threading
+        self.rows, self.stop_flag, self.err = [], False, None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
-                                      stdout=self.f, stderr=subprocess.DEVNULL)
-        except Exception:
-            self.p = None
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv = nv
+            self.h = nv.nvmlDeviceGetHandleByIndex(index)
+            self.max = float(nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM))
+        except Exception as e:      # no NVML: report no samples rather than invent them
+            self.nv, self.err = None, repr(e)
+            return
+        self.t = threading.Thread(target=self._run, daemon=True)
+        self.t.start()
+
+    def _run(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.rows.append((float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)),
+                                  nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0,
+                                  int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                                  if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons")
+                                  else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))))
+            except Exception as e:
+                self.err = repr(e)
+                break
+            time.sleep(0.005)
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.p is None:
+        if self.nv is None:
+            out["error"] = self.err
             return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except Exception:
-            self.p.kill()
-        self.f.flush(); self.f.seek(0)
-        sm, mx, reasons, pw = [], [], set(), []
-        for line in self.f:
-            t = [x.strip() for x in line.split(",")]
-            if len(t) < 9:
-                continue
-            try:
-                sm.append(float(t[1])); mx.append(float(t[2])); pw.append(float(t[3]))
-            except ValueError:
-                continue
-            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), t[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        self.f.close()
-        os.unlink(self.f.name)
-        if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
-                       samples=len(sm), power_w_max=float(max(pw)))
+        self.stop_flag = True
+        self.t.join(timeout=2)
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        if self.rows:
+            allr = 0
+            for _, _, r in self.rows:
+                allr |= r
+            out.update(sm_mhz=float(np.median([r[0] for r in self.rows])), sm_max_mhz=self.max,
+                       reasons=sorted(k for k, bit in names.items() if allr & bit), samples=len(self.rows),
+                       power_w_max=float(max(r[1] for r in self.rows)))
         return out
 
 
@@ -157,6 +167,21 @@ def cpu_oracle_rate(name, size, seconds=10.0, dtype="f64"):
         n += 1
     dt = time.perf_counter() - t0
     return upd * n / dt, cores, sample + ", %d steps in %.1f s" % (n, dt), dt / n
+
+
+def max_over_ranks(x, dist=None, device="cpu"):
+    """Multi-GPU timing rule: every duration is the MAX over ranks (one process per GPU)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank_step, world, steps, ms):
+    """Weak scaling over independent replicas: units all ranks processed / the slowest rank's time."""
+    return units_per_rank_step * world * steps / (ms * 1e-3)
 
 
 def run_reference(args):
@@ -249,12 +274,9 @@ def run_ours(args):
     ms = t0.elapsed_time(t1)
     clocks = sampler.stop() if sampler else {}
     launches = g.get_counter(binding.CNT_LAUNCHES)
-    if dist is not None:
-        tt = torch.tensor([ms], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     ms_per_step = ms / args.steps
-    value = upd_per_step * world * args.steps / (ms * 1e-3)
+    value = whole_job_rate(upd_per_step, world, args.steps, ms)
 
     # finiteness of the state after the timed run (S4 warning): sample the first patches
     chk = g.download(0, 0, min(npatch, 64))
@@ -271,7 +293,7 @@ def run_ours(args):
         avg_ms = 0.5 * (s1 + s2)
         ach = 0.5 * (b1 + b2) / (avg_ms * 1e-3) / 1e9
         key = "%s_%s" % (args.workload, args.dtype)
-        roof = {"bound": "hbm", "kernel": {0: "k_rk_stage_ref", 1: "k_rk_stage_tile", 2: "k_rk_stage_march"}[args.kernel],
+        roof = {"bound": "hbm", "kernel": {0: "k_rk_stage_ref", 1: "k_rk_stage_tile", 2: "k_rk_stage_march", 3: "k_rk_stage_lite", 4: "k_rk_stage_quad"}[args.kernel],
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": NCU_TRAFFIC.get(key), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": 0.5 * (b1 + b2),
@@ -279,6 +301,20 @@ def run_ours(args):
                 "stage2": {"ms": s2, "GB/s": b2 / (s2 * 1e-3) / 1e9, "bytes_per_cell": 3 * nv * esz},
                 "share_of_step": (s1 + s2) / ms_per_step,
                 "frac_of_nominal_8TBs": ach / 8000.0}
+        # the arithmetic side of the same kernel: executed thread-instructions
+        # per cell and stage from the committed ncu capture / the SM's issue and FP64-pipe rates
+        ipc = (NCU_TRAFFIC.get("instr_per_cell_stage") or {}).get(key)
+        if ipc:
+            clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
+            alu = {"bound": "alu", "unit": "G thread-instr/s", "sm_mhz": clk / 1e6,
+                   "issue": {"instr_per_cell_stage": ipc["total"], "achieved": ipc["total"] * cells / (avg_ms * 1e-3) / 1e9,
+                             "peak": 148 * 128 * clk / 1e9}}
+            alu["issue"]["frac"] = alu["issue"]["achieved"] / alu["issue"]["peak"]
+            if "fp64" in ipc:
+                alu["fp64_pipe"] = {"instr_per_cell_stage": ipc["fp64"], "achieved": ipc["fp64"] * cells / (avg_ms * 1e-3) / 1e9,
+                                    "peak": 148 * 64 * clk / 1e9}
+                alu["fp64_pipe"]["frac"] = alu["fp64_pipe"]["achieved"] / alu["fp64_pipe"]["peak"]
+            roof["alu"] = alu
 
     # end to end through the C ABI with host buffers (H2D of all interiors, one step, D2H)
     e2e = None
@@ -292,11 +328,8 @@ def run_ours(args):
             g.advance_host(cfl, 0.0, 1, host_in.data_ptr(), host_out.data_ptr())
         torch.cuda.synchronize()
         el = time.perf_counter() - t0
-        if dist is not None:
-            tt = torch.tensor([el], device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            el = float(tt.item())
-        e2e = {"value": upd_per_step * world * args.e2e_steps / el, "unit": "cell-updates/s",
+        el = max_over_ranks(el, dist, "cuda")
+        e2e = {"value": whole_job_rate(upd_per_step, world, args.e2e_steps, el * 1e3), "unit": "cell-updates/s",
                "h2d_bytes_per_step": hb, "d2h_bytes_per_step": hb, "steps": args.e2e_steps,
                "api": "amrhydro_advance_host (pinned host buffers)"}
         finite = finite and bool(np.isfinite(host_out.numpy()[:8]).all())

@@ -49,7 +49,11 @@ extern "C" {
 #define AMRHYDRO_OPT_EINT_FLOOR 4 /* S11, default 1e-30; any time                                  */
 #define AMRHYDRO_OPT_KERNEL 5     /* rk_stage variant: 0 = reference one-thread-per-cell kernel,
                                      1 = z-marching shared-memory kernel (first version),
-                                     2 = TMA-fed z-marching kernel (default); any time            */
+                                     2 = TMA-fed z-marching kernel (default),
+                                     3 = its register-light variant (two CTAs per SM),
+                                     4 = the same on quarter-patch 8x8 tiles (3-warp CTAs);
+                                     3 and 4 are measured alternatives (profiles/README.md),
+                                     all five agree to round-off; any time                         */
 #define AMRHYDRO_OPT_HALO 6       /* 0 = rk_stage reads materialised ghost zones (default);
                                      1 = rk_stage reads sibling interiors directly, fill_ghosts
                                      then only writes coarse-fine / physical faces; any time      */

@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_DIR, "libamrhydro.so")
+# AMRHYDRO_LIB: an alternative build of the same library (kernel tuning variants)
+_SO = os.environ.get("AMRHYDRO_LIB") or os.path.join(_DIR, "libamrhydro.so")
 
 OPT_DTYPE, OPT_THETA, OPT_RHO_FLOOR, OPT_EINT_FLOOR, OPT_KERNEL, OPT_HALO = 1, 2, 3, 4, 5, 6
 CNT_LAUNCHES, CNT_FLOOR_HITS = 1, 2

@@ -17,12 +17,16 @@ def nvcc():
     return "nvcc"
 
 
-def build(force=False, verbose=False):
+def build(force=False, verbose=False, out=None, extra=()):
+    """extra: additional nvcc flags (tuning macros, e.g. -DAMR_MINB64=2); out: alternative .so path."""
+    global OUT
+    if out:
+        OUT, force = out, True
     if not force and os.path.exists(OUT) and all(os.path.getmtime(OUT) >= os.path.getmtime(d) for d in DEPS):
         return OUT
     cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "--use_fast_math" if os.environ.get("AMRHYDRO_FAST_MATH") else "-DAMRHYDRO_PRECISE",
-           "-Xcompiler", "-fPIC", "-shared", "-o", OUT, SRC]
+           "-Xcompiler", "-fPIC", "-shared", "-o", OUT, SRC] + list(extra)
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
@@ -31,5 +35,8 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    build(force=True, verbose="-v" in sys.argv)
+    a = [x for x in sys.argv[1:] if x != "-v"]
+    o = a[a.index("-o") + 1] if "-o" in a else None
+    ex = [x for x in a if x.startswith("-D")]
+    build(force=True, verbose="-v" in sys.argv, out=o, extra=ex)
     print(OUT)

@@ -18,6 +18,8 @@
 #include "rk_stage_ref.cuh"
 #include "rk_stage_tile.cuh"
 #include "rk_stage_march.cuh"
+#include "rk_stage_lite.cuh"
+#include "rk_stage_quad.cuh"
 
 using namespace amr;
 
@@ -46,7 +48,8 @@ struct amrhydro {
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
-  CUtensorMap tmap;            // TMA view of the pool (rk_stage_march)
+  CUtensorMap tmap;            // TMA view of the pool, 16x16 boxes (rk_stage_march)
+  CUtensorMap tmap8;           // the same with 8x8 boxes (rk_stage_quad)
   bool have_tmap = false;
   std::string err;
 };
@@ -173,7 +176,7 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
       (key == AMRHYDRO_OPT_RHO_FLOOR ? h->rho_floor : h->e_floor) = value;
       return 0;
     case AMRHYDRO_OPT_KERNEL:
-      if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0, 1 or 2");
+      if (value < 0 || value > 4 || value != int(value)) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0..4");
       h->kernel = int(value);
       return 0;
     case AMRHYDRO_OPT_HALO:
@@ -219,7 +222,8 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   {
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      return make_tensor_map<T, decltype(nv)::value>(&h->tmap, dev_pool, size_t(max_patches), nslots);
+      int e = make_tensor_map<T, decltype(nv)::value>(&h->tmap, dev_pool, size_t(max_patches), nslots);
+      return e ? e : make_tensor_map<T, decltype(nv)::value>(&h->tmap8, dev_pool, size_t(max_patches), nslots, 8);
     });
     h->have_tmap = (r == 0);
     if (r) { h->bound = false; return fail(h, AMRHYDRO_ECUDA, "cuTensorMapEncodeTiled failed for the pool"); }
@@ -455,6 +459,16 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
                                                                 T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
+      LAUNCH_CHECK(h);
+    } else if (h->kernel == 4) {
+      int r = launch_rk_stage_quad<T, NV>(h->tmap8, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_quad: ") + cudaGetErrorString((cudaError_t)r));
+      LAUNCH_CHECK(h);
+    } else if (h->kernel == 3) {
+      int r = launch_rk_stage_lite<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_lite: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
     } else if (h->kernel == 2) {
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),

@@ -113,7 +113,7 @@ def test_fill_ghosts_prolongation_matches_oracle(gpu, kind, alpha):
 # ------------------------------------------------------------------ a3-a6: one stage
 @pytest.mark.parametrize("nv", [5, 8])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("kernel,halo", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1)])
+@pytest.mark.parametrize("kernel,halo", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1), (4, 0), (4, 1)])
 def test_rk_stage_matches_oracle(gpu, nv, dtype, kernel, halo):
     h = wl.uniform_hierarchy(2, periodic=True)
     g, o = make_pair(gpu, h, 5.0 / 3.0, nv, dtype, kernel=kernel, halo=halo)
@@ -143,7 +143,7 @@ def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
     h = wl.uniform_hierarchy(2, periodic=False)
     U = rand_state(h, 5, 8)
     res = []
-    for kernel, halo in ((0, 0), (1, 0), (1, 1), (2, 0), (2, 1)):
+    for kernel, halo in ((0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1), (4, 0), (4, 1)):
         g = gpu.AmrHydro(h, 1.4, 5, kernel=kernel, halo=halo)
         g.upload(0, U)
         g.fill_ghosts(0, 0)
@@ -153,6 +153,10 @@ def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
     assert norm_err(res[3], res[0]).max() <= 1e-14
     assert np.array_equal(res[1], res[2])      # halo source does not change the arithmetic
     assert np.array_equal(res[3], res[4])
+    assert norm_err(res[5], res[0]).max() <= 1e-14
+    assert np.array_equal(res[5], res[6])
+    assert norm_err(res[7], res[0]).max() <= 1e-14
+    assert np.array_equal(res[7], res[8])
 
 
 def test_uniform_state_bitwise_on_gpu(gpu):
