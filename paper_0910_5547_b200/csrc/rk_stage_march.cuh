@@ -186,6 +186,16 @@ __device__ __forceinline__ void face_flux(const T (&L)[8], const T (&R)[8], cons
   for (int v = 0; v < 8; ++v) G[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
 }
 
+// fp32: the same value from the 3-input min/max of sm_100 (FMNMX3): with x = 2 theta dm, y = 2 theta dp,
+// lo = min(x, y, c) <= hi = max(x, y, c), the minmod is the median of (0, lo, hi) = max(lo, min(0, hi))
+// -- 6 instructions instead of 9, none of them a select.  (fp64 has no native min/max: it keeps
+// the compare/select form above.)
+__device__ __forceinline__ float slope4(float dm, float dp, float c, float theta2) {
+  const float x = theta2 * dm, y = theta2 * dp;
+  const float lo = fminf(fminf(x, y), c), hi = fmaxf(fmaxf(x, y), c);
+  return fmaxf(lo, fminf(0.f, hi));
+}
+
 // ---- TMA / mbarrier (PTX ISA: cp.async.bulk.tensor, mbarrier)
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {

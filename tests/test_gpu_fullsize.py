@@ -53,7 +53,8 @@ def check_fullsize(gpu, G, gamma, nv, dtype, nsample, seed, tol, cfl=0.3):
     org = np.asarray(h["origin"]) // 16
     rng = np.random.default_rng(seed)
     picks = list(rng.choice(len(org), size=nsample - 2, replace=False)) + [0, len(org) - 1]   # incl. wrap-around patches
-    hb = wl.uniform_hierarchy(3, periodic=True, order="linear")
+    hb = wl.build_hierarchy((3, 3, 3), (), (0,) * 6, box=48.0 / n, order="linear")   # periodic, same cell size as the full level
+    assert abs(hb["dx0"] - 1.0 / n) < 1e-15 / n
     ob = np.asarray(hb["origin"]) // 16
     centre = int(np.where((ob == 1).all(axis=1))[0][0])
     smax, worst = 0.0, 0.0
