@@ -319,7 +319,7 @@ def run_ours(args):
     # end to end through the C ABI with host buffers (H2D of all interiors, one step, D2H)
     e2e = None
     if not args.no_e2e:
-        host_out = torch.empty_like(host_in)
+        host_out = torch.empty(host_in.shape, dtype=host_in.dtype, pin_memory=True)   # (empty_like would drop the pinning)
         hb = npatch * nv * 4096 * esz
         g.advance_host(cfl, 0.0, 1, host_in.data_ptr(), host_out.data_ptr())      # warm-up
         barrier()
