@@ -40,6 +40,7 @@ struct amrhydro {
   int bc[6] = {0, 0, 0, 0, 0, 0};
   std::vector<amrhydro_patch_desc> tbl;
   std::vector<int> child, octant, lev_first, lev_count;
+  std::vector<char> lev_has_cf, lev_has_phys;   // level has coarse-fine ghost regions / faces on an outflow boundary
   Desc *d_desc = nullptr;
   int *d_child = nullptr, *d_octant = nullptr;
   void *d_Rf = nullptr, *d_Rc = nullptr, *d_bflux = nullptr;
@@ -277,6 +278,14 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
   h->child = child; h->octant = octant; h->lev_first = first; h->lev_count = count;
   h->nlev = nlev; h->dx0 = dx0;
   for (int i = 0; i < 6; ++i) h->bc[i] = bc[i];
+  h->lev_has_cf.assign(nlev, 0);
+  h->lev_has_phys.assign(nlev, 0);
+  for (int p = 0; p < np; ++p) {
+    for (int r = 0; r < 27; ++r)
+      if (r != 13 && tbl[p].nbr[r] == -1) h->lev_has_cf[tbl[p].level] = 1;
+    for (int f = 0; f < 6; ++f)
+      if (tbl[p].nbr[face_region(f)] == -2 && bc[f] == AMRHYDRO_BC_OUTFLOW) h->lev_has_phys[tbl[p].level] = 1;
+  }
   CUDA_TRY(h, cudaMalloc(&h->d_desc, size_t(np) * sizeof(Desc)));
   CUDA_TRY(h, cudaMalloc(&h->d_child, size_t(np) * 8 * sizeof(int)));
   CUDA_TRY(h, cudaMalloc(&h->d_octant, size_t(np) * sizeof(int)));
@@ -428,18 +437,21 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
   }
   // direct-halo mode: sibling copies are only needed where someone prolongates from this level
   const int skip = (h->halo == 1 && level + 1 >= h->nlev) ? 1 : 0;
-  if (skip && h->nlev == 1) {
-    bool phys = false;
-    for (int f = 0; f < 6; ++f) phys |= (h->bc[f] == AMRHYDRO_BC_OUTFLOW);
-    if (!phys) return 0;   // periodic single level: nothing to materialise
-  }
+  const bool phase1 = !skip || h->lev_has_cf[level], phase2 = h->lev_has_phys[level];
+  if (!phase1 && !phase2) return 0;   // e.g. periodic single level with direct halos: nothing to materialise
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    k_fill_ghosts<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(
-        make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->bc[0], h->bc[1],
-        h->bc[2], h->bc[3], h->bc[4], h->bc[5], skip);
-    LAUNCH_CHECK(h);
+    if (phase1) {
+      k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
+          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, skip);
+      LAUNCH_CHECK(h);
+    }
+    if (phase2) {
+      k_fill_outflow<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(
+          make_pool<T>(h), slot, h->lev_first[level], h->d_desc, h->bc[0], h->bc[1], h->bc[2], h->bc[3], h->bc[4], h->bc[5]);
+      LAUNCH_CHECK(h);
+    }
     return 0;
   });
 }

@@ -87,17 +87,18 @@ template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
   return T(0);
 }
 
-// One block per patch.  Phase 1: every ghost cell whose 16^3 neighbour block is a sibling is
+// Phase 1 (k_fill_ghosts): one block per (patch, padded z-plane), so that even a level of a few
+// dozen patches fills the machine.  Every ghost cell whose 16^3 neighbour block is a sibling is
 // copied from that sibling's interior; where it is a coarse-fine boundary it is prolongated
 // from the parent's padded box, conservative limited-linear (S6) in time-interpolated parent
-// data (S7).  Phase 2: zero-gradient outflow, x then y then z over the full padded extent.
-// skip_siblings: face/edge/corner copies are skipped (rk_stage reads siblings directly).
+// data (S7; alpha = 0 or 1 reads only the slot that counts, which is the same value bitwise for
+// finite data).  skip_siblings: face/edge/corner copies are skipped (rk_stage reads siblings directly).
+// Phase 2 (k_fill_outflow, launched only for levels that touch an outflow boundary): zero-gradient
+// outflow, x then y then z over the full padded extent, one block per patch.
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
-                                                     int first, const Desc *__restrict__ desc,
-                                                     int bc0, int bc1, int bc2, int bc3, int bc4, int bc5,
-                                                     int skip_siblings) {
-  const int p = first + blockIdx.x;
+                                                     int first, const Desc *__restrict__ desc, int skip_siblings) {
+  const int p = first + blockIdx.x, k = blockIdx.y;
   const Desc &D = desc[p];
   T *U = pool.patch(slot, p);
   __shared__ int s_nbr[27];
@@ -111,13 +112,18 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   const int Q = D.parent;
   const T *Co = Q >= 0 ? pool.patch(pold, Q) : nullptr;
   const T *Cn = Q >= 0 ? pool.patch(pnew, Q) : nullptr;
-  for (int c = threadIdx.x; c < NP * NP * NP; c += 256) {
-    const int i = c % NP, j = (c / NP) % NP, k = c / (NP * NP);
+  const bool only_old = alpha == T(0), only_new = alpha == T(1);
+  const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
+  // ghost cells of this plane: all 400 on a z-ghost plane, else the 144 of the frame
+  const int ncell = oz != 0 ? NP * NP : NP * NP - NI * NI;
+  for (int t = threadIdx.x; t < ncell; t += 256) {
+    int i, j;
+    if (oz != 0) { i = t % NP; j = t / NP; }
+    else if (t < 2 * NG * NP) { i = t % NP; j = t / NP; if (j >= NG) j += NI; }      // rows 0,1,18,19
+    else { const int u = t - 2 * NG * NP; j = NG + u / (2 * NG); i = u % (2 * NG); if (i >= NG) i += NI; }
     const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0);
     const int oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
-    const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
     const int r = (oz + 1) * 9 + (oy + 1) * 3 + (ox + 1);
-    if (r == 13) continue;
     const int nb = s_nbr[r];
     const int me = cell<T>(k, j, i);
     if (nb >= 0) {
@@ -142,18 +148,33 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
         const T *o = Co + size_t(v) * Layout<T>::VS, *n = Cn + size_t(v) * Layout<T>::VS;
-        const T uc = (T(1) - alpha) * o[c0] + alpha * n[c0];
+        auto at = [&](int c) {
+          if (only_old) return o[c];
+          if (only_new) return n[c];
+          return (T(1) - alpha) * o[c] + alpha * n[c];
+        };
+        const T uc = at(c0);
         T val = uc;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-          const T up = (T(1) - alpha) * o[c0 + st[d]] + alpha * n[c0 + st[d]];
-          const T um = (T(1) - alpha) * o[c0 - st[d]] + alpha * n[c0 - st[d]];
+          const T up = at(c0 + st[d]);
+          const T um = at(c0 - st[d]);
           val = val + s[d] * minmod2(up - uc, uc - um);
         }
         U[size_t(v) * Layout<T>::VS + me] = val;
       }
     }
   }
+}
+
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_fill_outflow(Pool<T> pool, int slot, int first, const Desc *__restrict__ desc,
+                                                      int bc0, int bc1, int bc2, int bc3, int bc4, int bc5) {
+  const int p = first + blockIdx.x;
+  T *U = pool.patch(slot, p);
+  __shared__ int s_nbr[27];
+  if (threadIdx.x < 27) s_nbr[threadIdx.x] = desc[p].nbr[threadIdx.x];
+  __syncthreads();
   const int bc[6] = {bc0, bc1, bc2, bc3, bc4, bc5};
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
