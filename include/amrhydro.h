@@ -57,6 +57,12 @@ extern "C" {
 #define AMRHYDRO_OPT_HALO 6       /* 0 = rk_stage reads materialised ghost zones (default);
                                      1 = rk_stage reads sibling interiors directly, fill_ghosts
                                      then only writes coarse-fine / physical faces; any time      */
+#define AMRHYDRO_OPT_FUSE_CFL 7   /* the combination stage (a != 0) of the default rk_stage kernel can also reduce
+                                     the max signal speed of the state it writes, so that the next
+                                     amrhydro_cfl_dt of that slot launches nothing: 0 = never, 1 = always,
+                                     2 (default) = in fp32 only, where it costs nothing (measured at 512^3:
+                                     fp32 step 6.89 -> 6.09 ms; fp64 step 14.72 -> 14.26 ms but the FP64-pipe
+                                     bound stage grows by 0.57 ms); any time                          */
 
 /* counters (amrhydro_get_counter) */
 #define AMRHYDRO_CNT_LAUNCHES 1   /* kernels launched by this handle since create / last reset */
@@ -117,7 +123,13 @@ int amrhydro_download_registers(amrhydro_t *h, int patch, double *host_fine, dou
 
 /* a1: dt = cfl * dx_level / max over interior cells and d of (|v_d| + c_d), c = sound speed
  * (S2) or fast magnetosonic speed along d (S3).  S4; the paper gives no CFL formula.
- * Synchronises.  AMRHYDRO_ENONFINITE if the maximum is NaN, inf or 0.  smax_out may be NULL. */
+ * Synchronises.  AMRHYDRO_ENONFINITE if the maximum is NaN, inf or 0.  smax_out may be NULL.
+ * The library remembers the maximum of (level, slot) until a call writes interior cells of that
+ * slot (upload, rk_stage, restrict, reflux, copy_slot), and rk_stage's combination stage can
+ * supply it (AMRHYDRO_OPT_FUSE_CFL): the same cells, the same formula, reduced where the state is
+ * produced; the reciprocal there is correct to 1 ulp, so dt may differ from the stand-alone
+ * reduction in the last bit.  The pool is private: data written into it behind the library's back
+ * is not seen. */
 int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_out, double *smax_out);
 
 /* a2: fill the ghost zones of every patch of `level` in `slot` (S5): same-level copy where

@@ -45,7 +45,10 @@ struct amrhydro {
   int *d_child = nullptr, *d_octant = nullptr;
   void *d_Rf = nullptr, *d_Rc = nullptr, *d_bflux = nullptr;
   size_t bflux_patches = 0;
-  unsigned long long *d_scalars = nullptr;  // [0] smax bits, [1] floor hits
+  unsigned long long *d_scalars = nullptr;  // [0] scratch, [1] floor hits
+  unsigned long long *d_smax = nullptr;     // per level: bits of the max signal speed of (level, smax_slot[level])
+  std::vector<int> smax_slot;               // slot the cached value belongs to, -1 = stale
+  int fuse_cfl = 2;                         // 0 never, 1 always, 2 = where it is free (fp32)
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
@@ -123,9 +126,16 @@ int ensure_stage(amrhydro *h, size_t bytes) {
   return 0;
 }
 
+// cached max signal speed of (level, slot) goes stale when interior cells of the slot are written
+void smax_touch(amrhydro *h, int level, int slot) {
+  if (level >= 0 && level < (int)h->smax_slot.size() && h->smax_slot[level] == slot) h->smax_slot[level] = -1;
+}
+
 void free_hierarchy(amrhydro *h) {
   cudaFree(h->d_desc); cudaFree(h->d_child); cudaFree(h->d_octant);
-  cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux);
+  cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux); cudaFree(h->d_smax);
+  h->d_smax = nullptr;
+  h->smax_slot.clear();
   h->d_desc = nullptr; h->d_child = h->d_octant = nullptr;
   h->d_Rf = h->d_Rc = h->d_bflux = nullptr;
   h->bflux_patches = 0;
@@ -184,6 +194,10 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
       if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "halo must be 0 or 1");
       h->halo = int(value);
       return 0;
+    case AMRHYDRO_OPT_FUSE_CFL:
+      if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "fuse_cfl must be 0, 1 or 2");
+      h->fuse_cfl = int(value);
+      return 0;
   }
   return fail(h, AMRHYDRO_EINVAL, "unknown option");
 }
@@ -220,6 +234,7 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   h->pool = dev_pool; h->pool_bytes = bytes; h->maxp = max_patches; h->nslots = nslots;
   h->stream = (cudaStream_t)stream;
   h->bound = true;
+  std::fill(h->smax_slot.begin(), h->smax_slot.end(), -1);
   {
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
@@ -286,6 +301,8 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
     for (int f = 0; f < 6; ++f)
       if (tbl[p].nbr[face_region(f)] == -2 && bc[f] == AMRHYDRO_BC_OUTFLOW) h->lev_has_phys[tbl[p].level] = 1;
   }
+  CUDA_TRY(h, cudaMalloc(&h->d_smax, size_t(nlev) * sizeof(unsigned long long)));
+  h->smax_slot.assign(nlev, -1);
   CUDA_TRY(h, cudaMalloc(&h->d_desc, size_t(np) * sizeof(Desc)));
   CUDA_TRY(h, cudaMalloc(&h->d_child, size_t(np) * 8 * sizeof(int)));
   CUDA_TRY(h, cudaMalloc(&h->d_octant, size_t(np) * sizeof(int)));
@@ -313,6 +330,7 @@ int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *h
   const size_t per = size_t(h->nv) * 4096 * elem(h);
   const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
   if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
+  for (int l = 0; l < h->nlev; ++l) smax_touch(h, l, slot);
   for (int done = 0; done < count; done += chunk) {
     int n = std::min(chunk, count - done);
     CUDA_TRY(h, cudaMemcpyAsync(h->d_stage, (const char *)host + size_t(done) * per, size_t(n) * per,
@@ -388,23 +406,36 @@ int amrhydro_download_registers(amrhydro_t *h, int patch, double *rf, double *rc
   return 0;
 }
 
-// enqueue the max-speed reduction of one level into d_scalars[0] (not reset here)
-static int enqueue_cfl(amrhydro_t *h, int level, int slot) {
-  return dispatch(h, [&](auto t, auto nv) {
+// The max signal speed of (level, slot) lives in d_smax[level].  It is produced either by k_cfl or,
+// for free, by the combination stage of rk_stage_march that wrote the slot (fused reduction), and it
+// goes stale whenever a call writes interior cells of that slot (upload, rk_stage, restrict, reflux,
+// copy_slot): smax_slot[level] records which slot the value describes.
+static int ensure_smax(amrhydro_t *h, int level, int slot) {
+  if (h->smax_slot[level] == slot) return 0;
+  CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
+  int r = dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
     k_cfl<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level],
-                                                              make_params<T>(h), h->d_scalars, h->d_scalars + 1);
+                                                              make_params<T>(h), h->d_smax + level, h->d_scalars + 1);
     LAUNCH_CHECK(h);
     return 0;
   });
+  if (r == 0) h->smax_slot[level] = slot;
+  return r;
 }
-static int read_smax(amrhydro_t *h, double *smax) {
-  unsigned long long bits = 0;
-  CUDA_TRY(h, cudaMemcpyAsync(&bits, h->d_scalars, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
+// max over levels [l0, l1] of the cached values (one small copy, one synchronisation)
+static int read_smax(amrhydro_t *h, int l0, int l1, double *smax) {
+  std::vector<unsigned long long> bits(h->nlev, 0);
+  CUDA_TRY(h, cudaMemcpyAsync(bits.data(), h->d_smax, size_t(h->nlev) * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                              h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-  double s;
-  std::memcpy(&s, &bits, sizeof(s));
+  double s = 0;
+  for (int l = l0; l <= l1; ++l) {
+    double v;
+    std::memcpy(&v, &bits[l], sizeof(v));
+    if (!(v <= s)) s = v;                  // keeps NaN/inf
+  }
   *smax = s;
   if (!(s > 0.0) || !std::isfinite(s)) return fail(h, AMRHYDRO_ENONFINITE, "max signal speed is zero or not finite");
   return 0;
@@ -415,10 +446,9 @@ int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_o
   if (int r = check_level(h, level)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (!dt_out) return fail(h, AMRHYDRO_EINVAL, "dt_out is null");
-  CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, sizeof(unsigned long long), h->stream));
-  if (int r = enqueue_cfl(h, level, slot)) return r;
+  if (int r = ensure_smax(h, level, slot)) return r;
   double s = 0;
-  int r = read_smax(h, &s);
+  int r = read_smax(h, level, level, &s);
   if (smax_out) *smax_out = s;
   if (r) return r;
   *dt_out = cfl * (h->dx0 / double(1 << level)) / s;
@@ -468,6 +498,7 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     constexpr int NV = decltype(nv)::value;
     const int n = h->lev_count[level], first = h->lev_first[level];
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
+    smax_touch(h, level, sout);
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
                                                                 T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
@@ -483,10 +514,15 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_lite: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
     } else if (h->kernel == 2) {
+      // the combination stage also reduces the max signal speed of what it writes (a1 fused into a6)
+      const bool fuse = (h->fuse_cfl == 1 || (h->fuse_cfl == 2 && h->bits == 32)) && a != 0.0;
+      if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                           make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+                                           make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
+                                           fuse ? h->d_smax + level : nullptr);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
+      if (fuse) h->smax_slot[level] = sout;
     } else {
       int r = launch_rk_stage_tile<T, NV>(make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                           make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
@@ -506,6 +542,7 @@ int amrhydro_restrict(amrhydro_t *h, int flev, int fslot, int cslot) {
   if (int r = check_ready(h)) return r;
   if (flev < 1 || flev >= h->nlev) return fail(h, AMRHYDRO_EINVAL, "fine_level out of range");
   if (check_slot(h, fslot) || check_slot(h, cslot)) return AMRHYDRO_EINVAL;
+  smax_touch(h, flev - 1, cslot);
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
@@ -521,6 +558,7 @@ int amrhydro_reflux(amrhydro_t *h, int clev, int slot) {
   if (int r = check_level(h, clev)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (clev + 1 >= h->nlev) return 0;
+  smax_touch(h, clev, slot);
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
@@ -539,6 +577,7 @@ int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {
   if (int r = check_level(h, level)) return r;
   if (check_slot(h, src) || check_slot(h, dst)) return AMRHYDRO_EINVAL;
   if (src == dst) return 0;
+  smax_touch(h, level, dst);
   const size_t per = size_t(h->nv) * vs(h) * elem(h);
   char *base = (char *)h->pool;
   CUDA_TRY(h, cudaMemcpyAsync(base + (size_t(dst) * h->maxp + h->lev_first[level]) * per,
@@ -572,11 +611,10 @@ int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out)
   if (h->nslots < (h->nlev > 1 ? 3 : 2)) return fail(h, AMRHYDRO_ESTATE, "advance needs 2 slots (3 with refinement)");
   double dt = dt_fixed;
   if (!(dt > 0.0)) {
-    CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, sizeof(unsigned long long), h->stream));
     for (int l = 0; l < h->nlev; ++l)
-      if (int r = enqueue_cfl(h, l, 0)) return r;
+      if (int r = ensure_smax(h, l, 0)) return r;
     double s = 0;
-    if (int r = read_smax(h, &s)) return r;
+    if (int r = read_smax(h, 0, h->nlev - 1, &s)) return r;
     dt = cfl * h->dx0 / s;                                  // S4: dt_l = dt0 / 2^l
   }
   if (dt_out) *dt_out = dt;

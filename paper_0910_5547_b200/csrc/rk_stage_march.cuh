@@ -196,6 +196,18 @@ __device__ __forceinline__ float slope4(float dm, float dp, float c, float theta
   return fmaxf(lo, fminf(0.f, hi));
 }
 
+// S4 for the fused CFL reduction: max_d |v_d| + c_d.  Euler: the MUFU-seeded square root of this file
+// (error ~1e-19 relative) instead of the IEEE one; MHD: the stand-alone formula of physics.cuh.
+template <typename T, int NV> __device__ __forceinline__ T max_speed_fast(const T (&W)[NV], const Params<T> &P) {
+  if (NV == 5) {
+    const T ax = tabs(W[2]), ay = tabs(W[3]), az = tabs(W[4]);
+    const T m1 = ax > ay ? ax : ay;
+    return (m1 > az ? m1 : az) + fsqrt(P.gg1 * W[1]);
+  } else {
+    return max_signal_speed<T, NV>(W, P);
+  }
+}
+
 // ---- TMA / mbarrier (PTX ISA: cp.async.bulk.tensor, mbarrier)
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
@@ -359,7 +371,7 @@ template <typename T, int NV, bool BASE>
 __global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : AMR_MINB32))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                 const Desc *__restrict__ desc, int direct_halo) {
+                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out) {
   using S = mk::Smem<T, NV>;
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
@@ -392,6 +404,8 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     T *qx = sm + S::O_QX + j * PQ + i, *fx = sm + S::O_FX + j * PQ + i;   // slot i: q+ of cell i-1 / flux at face i
     T *qy = sm + S::O_QY + j * PY + i, *fy = sm + S::O_FY + j * PY + i;
     T Wc[NV], dzm[NV], qpz[NV], acc[NV];
+    T best = T(0);                      // fused CFL reduction (a1) over the cells this thread finishes
+    bool bad = false;
     {
       T U0[NV], U1[NV], U2[NV], W0[NV], W1[NV];
       mk::mbar_wait(&bars[0], 0);
@@ -466,10 +480,22 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         const T *ui = raw + ((c - 1) % S::NSLOT) * RAWP;     // raw U of cell c-1 is still in the ring
         T *o = out + (c - 1) * PLANE;
 #pragma unroll
+        T un[NV];
+#pragma unroll
         for (int v = 0; v < NV; ++v) {
           T pre = b * ui[v * (NI * NI)];
           if (BASE) pre = fma(a, ub[v], pre);
-          o[size_t(v) * VS] = fma(-kk, acc[v] + Gz[v], pre);        // Eq. 7-8
+          un[v] = fma(-kk, acc[v] + Gz[v], pre);                    // Eq. 7-8
+          o[size_t(v) * VS] = un[v];
+        }
+        if (BASE && smax_out) {
+          // S4 on the state just produced: max_d |v_d| + c_d, with the NaN/inf test of k_cfl
+          T Wq[NV];
+          mk::prim<T, NV>(un, Wq, P, hits);
+          const T sp = mk::max_speed_fast<T, NV>(Wq, P);
+          const T chk = ((Wq[2] + Wq[3]) + Wq[4]) + sp;
+          bad |= !(chk - chk == T(0));
+          best = tmax(best, sp);
         }
       }
       if (c < NG + NI) {
@@ -519,6 +545,13 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
       }
 #pragma unroll
       for (int v = 0; v < NV; ++v) Wc[v] = Wn[v];
+    }
+    if (BASE && smax_out) {
+      // one atomicMax per warp on the bit pattern of a non-negative double (monotone as an unsigned integer)
+      double bq = bad ? __longlong_as_double(0x7ff0000000000000LL) : double(best);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) bq = fmax(bq, __shfl_xor_sync(0xffffffffu, bq, o));
+      if (lane == 0) atomicMax(smax_out, (unsigned long long)__double_as_longlong(bq));
     }
   } else {
     // ------------------------------------------------------------------ halo warps (+ TMA producer)
@@ -575,7 +608,7 @@ int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int ns
 template <typename T, int NV>
 int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                          cudaStream_t stream) {
+                          cudaStream_t stream, unsigned long long *smax_out = nullptr) {
   static bool configured = false;
   constexpr size_t bytes = mk::Smem<T, NV>::BYTES;
   if (!configured) {
@@ -587,10 +620,10 @@ int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sb
   }
   if (a != T(0))
     k_rk_stage_march<T, NV, true><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
-                                                                     floor_hits, desc, direct_halo);
+                                                                     floor_hits, desc, direct_halo, smax_out);
   else
     k_rk_stage_march<T, NV, false><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
-                                                                      floor_hits, desc, direct_halo);
+                                                                      floor_hits, desc, direct_halo, nullptr);
   return 0;
 }
 

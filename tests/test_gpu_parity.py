@@ -57,6 +57,49 @@ def test_cfl_dt_matches_oracle(gpu, nv, dtype):
     assert abs(g.cfl_dt(0, 0, 0.3) - o.cfl_dt(0, 0, 0.3)) <= tol * o.cfl_dt(0, 0, 0.3)
 
 
+@pytest.mark.parametrize("nv,dtype", [(5, "f64"), (8, "f64"), (5, "f32")])
+def test_cfl_fused_into_combination_stage(gpu, nv, dtype):
+    """a1 fused into a6 (AMRHYDRO_OPT_FUSE_CFL): same dt as the stand-alone reduction and as the
+    oracle, no kernel launched by cfl_dt, and the cached value goes stale when the slot is written."""
+    h = wl.uniform_hierarchy(2, periodic=True)
+    U = rand_state(h, nv, 21)
+    res = {}
+    for fuse in (1, 0):
+        g, o = make_pair(gpu, h, 1.4, nv, dtype, halo=1, fuse_cfl=fuse)
+        upload_both(g, o, U, dtype)
+        dt = 0.3 * o.cfl_dt(0, 0, 1.0)
+        for x in (g, o):
+            x.fill_ghosts(0, 0)
+            x.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
+            x.fill_ghosts(0, 1)
+            x.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+        n0 = g.get_counter(gpu.CNT_LAUNCHES)
+        res[fuse] = g.cfl_dt(0, 0, 0.3)
+        assert g.get_counter(gpu.CNT_LAUNCHES) - n0 == (0 if fuse else 1)
+        tol = 1e-14 if dtype == "f64" else 2e-6
+        assert abs(res[fuse] - o.cfl_dt(0, 0, 0.3)) <= tol * res[fuse]
+        if fuse:
+            V = U.copy()
+            V[:, 1:4] *= 3.0                       # faster flow, same slot: the cached maximum must not survive
+            V[:, 4] += 4.0 * (U[:, 1:4] ** 2).sum(axis=1) / U[:, 0]
+            upload_both(g, o, V, dtype)
+            d2 = g.cfl_dt(0, 0, 0.3)
+            assert abs(d2 - o.cfl_dt(0, 0, 0.3)) <= tol * d2 and d2 < 0.9 * res[1]
+    assert abs(res[0] - res[1]) <= (1e-14 if dtype == "f64" else 2e-6) * res[0]
+
+
+def test_cfl_fused_reports_nonfinite(gpu):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g = gpu.AmrHydro(h, 1.4, 5, halo=1)
+    U = rand_state(h, 5, 22)
+    U[3, 0, 5, 6, 7] = np.nan
+    g.upload(0, U)
+    g.fill_ghosts(0, 0)
+    g.rk_stage(0, 0, 0, 1, 0.5, 0.5, 1e-3)
+    with pytest.raises(gpu.AmrHydroError):
+        g.cfl_dt(0, 1, 0.3)
+
+
 def test_cfl_dt_reports_nonfinite(gpu):
     h = wl.uniform_hierarchy(1, periodic=True)
     g = gpu.AmrHydro(h, 1.4, 5)
