@@ -68,6 +68,13 @@ def lib():
         L.orc_face.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int] + [dp] * 7
         L.orc_prim.argtypes = [C.c_int, C.c_double, dp, dp]
         L.orc_flux.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, dp, dp]
+        L.orc_set_glm.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.orc_set_glm.restype = None
+        L.orc_glm_damp.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double]
+        L.orc_flux_glm.argtypes = [C.c_double, C.c_double, C.c_int, dp, dp, dp]
+        L.orc_flux_glm.restype = None
+        L.orc_riemann_glm.argtypes = [C.c_double, C.c_double, C.c_int, dp, dp, dp]
+        L.orc_riemann_glm.restype = C.c_double
         _lib = L
     return _lib
 
@@ -108,11 +115,28 @@ def flux(nvars, gamma, direction, W):
     return U, F, c.value
 
 
+def flux_glm(gamma, ch, direction, W):
+    """(U(W), F^d(W)) of one 9-variable GLM-MHD primitive state (Eq. 14-15)."""
+    W = np.ascontiguousarray(W, dtype=np.float64)
+    U, F = np.zeros(9), np.zeros(9)
+    lib().orc_flux_glm(gamma, ch, direction, _dp(W), _dp(U), _dp(F))
+    return U, F
+
+
+def riemann_glm(gamma, ch, direction, WL, WR):
+    """Eq. 12 between two given 9-variable states.  Returns (lambda0, F)."""
+    WL, WR = (np.ascontiguousarray(x, dtype=np.float64) for x in (WL, WR))
+    F = np.zeros(9)
+    lam = lib().orc_riemann_glm(gamma, ch, direction, _dp(WL), _dp(WR), _dp(F))
+    return lam, F
+
+
 class Oracle:
-    """One hierarchy + pool held by the C++ oracle.  Slots: 0=A, 1=B, 2=C."""
+    """One hierarchy + pool held by the C++ oracle.  Slots: 0=A, 1=B, 2=C.
+    nvars = 9: GLM-MHD with wave speed ch and damping ratio cr = c_p^2/c_h (0 = no damping)."""
 
     def __init__(self, hier, gamma, nvars, bits=64, theta=1.5, rho_floor=1e-30, e_floor=1e-30,
-                 nslots=3, threads=1):
+                 nslots=3, threads=1, ch=1.0, cr=0.18):
         L = lib()
         self.h = L.orc_create(bits, gamma, nvars, theta, rho_floor, e_floor)
         if not self.h:
@@ -126,6 +150,8 @@ class Oracle:
         if r:
             raise ValueError("orc_set_hierarchy failed: %d" % r)
         L.orc_set_threads(self.h, threads)
+        if nvars == 9:
+            L.orc_set_glm(self.h, ch, cr)
 
     def __del__(self):
         if getattr(self, "h", None):
@@ -187,6 +213,9 @@ class Oracle:
     def reflux(self, coarse_level, slot=0):
         if lib().orc_reflux(self.h, coarse_level, slot):
             raise ValueError("reflux: improper nesting")
+
+    def glm_damp(self, level, slot, factor):
+        lib().orc_glm_damp(self.h, level, slot, factor)
 
     def copy_slot(self, level, src, dst):
         lib().orc_copy_slot(self.h, level, src, dst)

@@ -19,10 +19,11 @@
 // Storage (private to the oracle): pool[slot][patch][var][k][j][i] over the padded
 // 20^3 box (2 ghost + 16 interior + 2 ghost per axis, i fastest).
 //
-// Variables (Eq. 2; Eq. 14 without psi = reading S3'):
-//   U = (rho, rho vx, rho vy, rho vz, rho E [+ B^2/2], [Bx, By, Bz])
+// Variables (Eq. 2; Eq. 14; 8 variables = Eq. 14 without psi, reading S3';
+// 9 variables = the GLM system the paper ran, readings S17-S19 of DESIGN.md):
+//   U = (rho, rho vx, rho vy, rho vz, rho E [+ B^2/2], [Bx, By, Bz], [psi])
 // Primitives handed to reconstruction ("Rho, Eint, Vx, Vy, Vz"):
-//   W = (rho, e, vx, vy, vz, [Bx, By, Bz])
+//   W = (rho, e, vx, vy, vz, [Bx, By, Bz], [psi])
 
 #include <algorithm>
 #include <array>
@@ -39,7 +40,7 @@ constexpr int NI = 16;          // interior cells per side (BASELINE.json north_
 constexpr int NG = 2;           // ghost zones per side (stencil i-2..i+1)
 constexpr int NP = NI + 2 * NG; // padded side = 20
 constexpr int NC = NP * NP * NP;
-constexpr int MAXV = 8;
+constexpr int MAXV = 9;
 
 inline int cidx(int k, int j, int i) { return (k * NP + j) * NP + i; }
 
@@ -61,12 +62,14 @@ template <class T> inline T minmod2(T a, T b) {
 }
 
 template <class T> struct Phys {
-  int nv;        // 5 Euler, 8 ideal MHD
+  int nv;        // 5 Euler, 8 ideal MHD, 9 GLM-MHD
   T gamma;       // PAPER.md:71 Eq. 6
   T theta;       // PAPER.md:110, reading S1
   T rho_floor;   // reading S11
   T e_floor;
   long *floor_hits;
+  T ch = T(0);   // c_h of Eq. 15, reading S17: a constant given by the caller
+  T cr = T(0);   // c_p^2 / c_h of Dedner et al. 2002 ("damping rate"), reading S18; 0 = no damping
 
   // O1: conserved -> primitive.  PAPER.md:59 (E = v^2/2 + e), PAPER.md:298 (energy slot rho E + B^2/2)
   inline void prim(const T *U, T *W) const {
@@ -74,11 +77,12 @@ template <class T> struct Phys {
     if (!(rho >= rho_floor)) { rho = rho_floor; if (floor_hits) ++*floor_hits; }
     T vx = U[1] / rho, vy = U[2] / rho, vz = U[3] / rho;
     T etot = U[4];
-    if (nv == 8) {
+    if (nv >= 8) {
       T B2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
       etot = etot - T(0.5) * B2;
       W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
     }
+    if (nv == 9) W[8] = U[8];
     T e = etot / rho - T(0.5) * (vx * vx + vy * vy + vz * vz);
     if (!(e >= e_floor)) { e = e_floor; if (floor_hits) ++*floor_hits; }
     W[0] = rho; W[1] = e; W[2] = vx; W[3] = vy; W[4] = vz;
@@ -95,11 +99,12 @@ template <class T> struct Phys {
     T v2 = vx * vx + vy * vy + vz * vz;
     U[0] = rho; U[1] = rho * vx; U[2] = rho * vy; U[3] = rho * vz;
     U[4] = rho * (T(0.5) * v2 + e);
-    if (nv == 8) {
+    if (nv >= 8) {
       T B2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
       U[4] = U[4] + T(0.5) * B2;
       U[5] = W[5]; U[6] = W[6]; U[7] = W[7];
     }
+    if (nv == 9) U[8] = W[8];
   }
 
   // physical flux F^d(W).  Euler: Eq. 3-5 PAPER.md:63-67.  MHD: Eq. 15
@@ -126,6 +131,10 @@ template <class T> struct Phys {
       F[4] = F[4] + B2 * vd - Bd * Bv;
       for (int i = 0; i < 3; ++i) F[5 + i] = vd * B[i] - Bd * v[i];
       F[5 + d] = T(0);                          // psi == 0 in the 8-variable system
+      if (nv == 9) {                            // Eq. 15: F^d(B_d) = psi, F^d(psi) = c_h^2 B_d
+        F[5 + d] = W[8];
+        F[8] = ch * ch * Bd;
+      }
     }
   }
 
@@ -169,6 +178,7 @@ template <class T> struct Phys {
     T lp = std::max(T(0), std::max(vl + cl, vr + cr));          // max(0, lambda_l^+, lambda_r^+)
     T lm = std::max(T(0), std::max(-(vl - cl), -(vr - cr)));    // max(0,-lambda_l^-,-lambda_r^-)
     T lam0 = std::max(lp, lm);
+    if (nv == 9) lam0 = std::max(lam0, ch);    // the (B_d, psi) pair travels at +-c_h (reading S17)
     for (int q = 0; q < nv; ++q) F[q] = T(0.5) * (FL[q] + FR[q] - lam0 * (UR[q] - UL[q]));
     return lam0;
   }
@@ -233,6 +243,7 @@ template <class T> struct Hier {
             q.prim(Uc, W);
             for (int d = 0; d < 3; ++d) {
               double sd = double(std::fabs(W[2 + d]) + q.speed(W, d));
+              if (nv == 9 && !(sd >= double(q.ch))) sd = double(q.ch);   // S17: c_h bounds the time step too
               if (!(sd <= s)) s = sd;  // NaN propagates
             }
           }
@@ -469,6 +480,18 @@ template <class T> struct Hier {
     return 0;
   }
 
+  // S18: the damping of psi in the mixed GLM form of Dedner et al. (2002), psi_t = ... - (c_h^2/c_p^2) psi,
+  // integrated exactly over one step of the level, operator-split after the step: psi *= factor.
+  void glm_damp(int lev, int slot, double factor) {
+    if (nv != 9) return;
+    for (int p : lev_patches[lev]) {
+      T *psi = P(slot, p) + size_t(8) * NC;
+      for (int k = NG; k < NG + NI; ++k)
+        for (int j = NG; j < NG + NI; ++j)
+          for (int i = NG; i < NG + NI; ++i) psi[cidx(k, j, i)] = psi[cidx(k, j, i)] * T(factor);
+    }
+  }
+
   void copy_slot(int lev, int src, int dst) {
     for (int p : lev_patches[lev]) std::memcpy(P(dst, p), P(src, p), patch_stride() * sizeof(T));
   }
@@ -484,6 +507,7 @@ template <class T> struct Hier {
     rk_stage(lev, 0, 0, 1, 0.0, 1.0, dt, w);             // U1 = Un + dt L(Un)
     fill_ghosts(lev, 1, 2, 0, a2);
     rk_stage(lev, 1, 0, 0, 0.5, 0.5, dt, w);             // Un+1 = 1/2 Un + 1/2 (U1 + dt L(U1))
+    if (nv == 9 && ph.cr > T(0)) glm_damp(lev, 0, std::exp(-dt * double(ph.ch) / double(ph.cr)));
     if (kids) {
       fill_ghosts(lev, 0, 2, 0, a2);                     // new-time ghosts for the children's prolongation
       if (advance(lev + 1, 0.5 * dt, 0.0, 0.5)) return -1;
@@ -557,7 +581,7 @@ int set_hierarchy(Hier<T> &H, int np, int nlev, const int *level, const int *ori
 extern "C" {
 
 void *orc_create(int bits, double gamma, int nvars, double theta, double rho_floor, double e_floor) {
-  if ((bits != 32 && bits != 64) || (nvars != 5 && nvars != 8)) return nullptr;
+  if ((bits != 32 && bits != 64) || (nvars != 5 && nvars != 8 && nvars != 9)) return nullptr;
   Handle *h = new Handle;
   h->bits = bits;
   if (bits == 64) {
@@ -574,6 +598,10 @@ void *orc_create(int bits, double gamma, int nvars, double theta, double rho_flo
 void orc_destroy(void *h) { Handle *H = (Handle *)h; delete H->d; delete H->f; delete H; }
 void orc_set_threads(void *h, int n) { DISPATCH(h, H.nthreads = n); }
 void orc_set_theta(void *h, double th) { DISPATCH(h, H.ph.theta = decltype(H.ph.theta)(th)); }
+void orc_set_glm(void *h, double ch, double cr) {
+  DISPATCH(h, { H.ph.ch = decltype(H.ph.ch)(ch); H.ph.cr = decltype(H.ph.cr)(cr); });
+}
+int orc_glm_damp(void *h, int lev, int slot, double factor) { DISPATCH(h, H.glm_damp(lev, slot, factor)); return 0; }
 long orc_floor_hits(void *h) { long r = 0; DISPATCH(h, r = H.floor_hits); return r; }
 
 int orc_set_hierarchy(void *h, int np, int nlev, const int *level, const int *origin, const int *parent,
@@ -664,5 +692,16 @@ void orc_prim(int nvars, double gamma, const double *U, double *W) {
 void orc_flux(int nvars, double gamma, int dir, const double *W, double *U, double *F, double *c) {
   Phys<double> q{nvars, gamma, 1.5, 1e-300, 1e-300, nullptr};
   q.cons(W, U); q.flux(W, dir, F); *c = q.speed(W, dir);
+}
+// the same for the 9-variable system with its c_h; face flux of Eq. 12 from two given states
+void orc_flux_glm(double gamma, double ch, int dir, const double *W, double *U, double *F) {
+  Phys<double> q{9, gamma, 1.5, 1e-300, 1e-300, nullptr};
+  q.ch = ch;
+  q.cons(W, U); q.flux(W, dir, F);
+}
+double orc_riemann_glm(double gamma, double ch, int dir, const double *WL, const double *WR, double *F) {
+  Phys<double> q{9, gamma, 1.5, 1e-300, 1e-300, nullptr};
+  q.ch = ch;
+  return q.riemann(WL, WR, dir, F);
 }
 }  // extern "C"

@@ -168,14 +168,16 @@ def join_global(h, U, l=0):
 
 
 # --------------------------------------------------------------------------- initial data
-def cons_from_prim(rho, p, v, gamma, B=None):
-    """U of Eq. 2 (Eq. 14 without psi when B is given) from primitive fields."""
+def cons_from_prim(rho, p, v, gamma, B=None, psi=None):
+    """U of Eq. 2 (Eq. 14 when B is given; its ninth slot when psi is given too) from primitive fields."""
     ke = 0.5 * rho * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
     E = p / (gamma - 1.0) + ke
     comps = [rho, rho * v[0], rho * v[1], rho * v[2], E]
     if B is not None:
         comps[4] = E + 0.5 * (B[0] ** 2 + B[1] ** 2 + B[2] ** 2)
         comps += [B[0], B[1], B[2]]
+        if psi is not None:
+            comps.append(psi)
     return np.stack([np.broadcast_to(c, np.shape(rho)).astype(np.float64) for c in comps])
 
 
