@@ -42,7 +42,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--workload", default="cfg5", choices=["cfg5", "cfg2", "cfg4", "cfg3"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg5", "cfg2", "cfg4", "cfg4g", "cfg3"])
     ap.add_argument("--size", type=int, default=0, help="cells per side (default: the config's own size)")
     ap.add_argument("--halo", type=int, default=1, help="1: rk_stage reads sibling interiors directly")
     ap.add_argument("--kernel", type=int, default=2)
@@ -56,6 +56,7 @@ WORKLOADS = {
     "cfg5": dict(size=512, gamma=1.4, nv=5, cfl=0.3, name="cfg5_euler_stress_512^3_periodic"),
     "cfg2": dict(size=256, gamma=5.0 / 3.0, nv=5, cfl=0.3, name="cfg2_kelvin_helmholtz_256^3_periodic"),
     "cfg4": dict(size=128, gamma=5.0 / 3.0, nv=8, cfl=0.3, name="cfg4_mhd_turbulence_128^3_periodic"),
+    "cfg4g": dict(size=128, gamma=5.0 / 3.0, nv=9, cfl=0.3, name="cfg4_glm_mhd_9var_128^3_periodic (NEXT-1: psi = 0 initially, c_h = 1, c_r = 0.18)"),
     "cfg3": dict(size=64, gamma=1.4, nv=5, cfl=0.3, name="cfg3_sedov_amr_64^3+4levels"),
 }
 
@@ -76,6 +77,8 @@ def make_workload(name, size, seed_shift=0):
         G = wl.kelvin_helmholtz_global(n, gamma=w["gamma"], seed=20002 + seed_shift)
     else:
         G = wl.mhd_turbulence_global(n, gamma=w["gamma"], seed=20004 + seed_shift)
+        if name == "cfg4g":
+            G = np.concatenate([G, np.zeros_like(G[:1])])
     U = wl.split_global(h, G)
     del G
     return h, U, n ** 3

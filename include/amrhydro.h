@@ -18,7 +18,8 @@
  *  - Pointers: `dev_*` are device pointers, `host_*` are host pointers (pageable or pinned).
  *  - Geometry: patch interior 16^3, 2 ghost zones, refinement ratio 2, cubic cells,
  *    dx_l = dx0 / 2^l.  nvars = 5 (Euler: rho, rho vx, rho vy, rho vz, rho E; PAPER.md:57
- *    Eq. 2) or 8 (ideal MHD: ... rho E + B^2/2, Bx, By, Bz; Eq. 14 without psi).
+ *    Eq. 2), 8 (ideal MHD: ... rho E + B^2/2, Bx, By, Bz; Eq. 14 without psi) or
+ *    9 (GLM-MHD: Eq. 14 with psi, fluxes Eq. 15, readings S17-S19).
  *  - Host-side patch data is always "interior" layout [var][16][16][16] (x fastest) of the
  *    element type selected by AMRHYDRO_OPT_DTYPE.  The pool's internal (padded, aligned)
  *    layout is private.
@@ -64,6 +65,10 @@ extern "C" {
                                      fp32 step 6.89 -> 6.09 ms; fp64 step 14.72 -> 14.26 ms but the FP64-pipe
                                      bound stage grows by 0.57 ms); any time                          */
 
+#define AMRHYDRO_OPT_GLM_CH 8     /* nvars = 9: c_h of Eq. 15 (S17), > 0, default 1; any time               */
+#define AMRHYDRO_OPT_GLM_CR 9     /* nvars = 9: c_r = c_p^2/c_h of the psi damping applied by amrhydro_advance
+                                     (S18), default 0.18, 0 = none; any time                               */
+
 /* counters (amrhydro_get_counter) */
 #define AMRHYDRO_CNT_LAUNCHES 1   /* kernels launched by this handle since create / last reset */
 #define AMRHYDRO_CNT_FLOOR_HITS 2 /* cells/states where a floor of S11 was applied (rk_stage, cfl) */
@@ -90,7 +95,7 @@ typedef struct amrhydro_patch_desc {
 } amrhydro_patch_desc;
 
 /* Create a solver context.  gamma: adiabatic index of Eq. 6, > 1.
- * nvars in {5, 8}; patch_dim must be 16 and nghost 2 (BASELINE.json north_star; the stencil
+ * nvars in {5, 8, 9}; patch_dim must be 16 and nghost 2 (BASELINE.json north_star; the stencil
  * i-2..i+1 of PAPER.md:104).  Returns NULL on a bad argument or when no CUDA device exists. */
 amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost);
 void amrhydro_destroy(amrhydro_t *h);
@@ -153,6 +158,11 @@ int amrhydro_restrict(amrhydro_t *h, int fine_level, int fine_slot, int coarse_s
 int amrhydro_reflux(amrhydro_t *h, int coarse_level, int slot);
 
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src_slot, int dst_slot);
+
+/* nvars = 9 only (AMRHYDRO_EINVAL otherwise): psi <- factor * psi on the interior cells of one level,
+ * the damping of the mixed GLM system of Dedner et al. 2002 adopted at PAPER.md:292 (S18);
+ * amrhydro_advance calls it after every step of a level with factor = exp(-dt_l c_h / c_r). */
+int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor);
 
 /* Host-side driver (bookkeeping only): one coarse step of the whole hierarchy with
  * ratio-2 subcycling (S9), slots 0/1/2 as above.  dt_fixed > 0 overrides the CFL step

@@ -13,7 +13,7 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 # AMRHYDRO_LIB: an alternative build of the same library (kernel tuning variants)
 _SO = os.environ.get("AMRHYDRO_LIB") or os.path.join(_DIR, "libamrhydro.so")
 
-OPT_DTYPE, OPT_THETA, OPT_RHO_FLOOR, OPT_EINT_FLOOR, OPT_KERNEL, OPT_HALO, OPT_FUSE_CFL = 1, 2, 3, 4, 5, 6, 7
+OPT_DTYPE, OPT_THETA, OPT_RHO_FLOOR, OPT_EINT_FLOOR, OPT_KERNEL, OPT_HALO, OPT_FUSE_CFL, OPT_GLM_CH, OPT_GLM_CR = 1, 2, 3, 4, 5, 6, 7, 8, 9
 CNT_LAUNCHES, CNT_FLOOR_HITS = 1, 2
 
 EXPORTS = [
@@ -21,7 +21,7 @@ EXPORTS = [
     "amrhydro_get_counter", "amrhydro_pool_bytes", "amrhydro_bind_pool", "amrhydro_set_hierarchy",
     "amrhydro_upload", "amrhydro_download", "amrhydro_download_padded", "amrhydro_download_registers",
     "amrhydro_cfl_dt", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
-    "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
+    "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
 ]
 
 
@@ -64,6 +64,7 @@ def load_library():
     L.amrhydro_restrict.argtypes = [vp, i, i, i]
     L.amrhydro_reflux.argtypes = [vp, i, i]
     L.amrhydro_copy_slot.argtypes = [vp, i, i, i]
+    L.amrhydro_glm_damp.argtypes = [vp, i, i, d]
     L.amrhydro_advance.argtypes = [vp, d, d, dp]
     L.amrhydro_advance_host.argtypes = [vp, d, d, i, vp, vp, dp]
     L.amrhydro_sync.argtypes = [vp]
@@ -79,7 +80,7 @@ class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
     def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=2, halo=0,
-                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2):
+                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():
             raise AmrHydroError("no CUDA device: the amrhydro path has no CPU fallback")
@@ -94,7 +95,8 @@ class AmrHydro:
         self.np_dtype = {"f64": np.float64, "f32": np.float32}[dtype]
         self._ok(self.L.amrhydro_set_option(self.h, OPT_DTYPE, 64.0 if dtype == "f64" else 32.0))
         for k, v in ((OPT_THETA, theta), (OPT_RHO_FLOOR, rho_floor), (OPT_EINT_FLOOR, e_floor),
-                     (OPT_KERNEL, kernel), (OPT_HALO, halo), (OPT_FUSE_CFL, fuse_cfl)):
+                     (OPT_KERNEL, kernel), (OPT_HALO, halo), (OPT_FUSE_CFL, fuse_cfl)) + \
+                (((OPT_GLM_CH, ch), (OPT_GLM_CR, cr)) if nvars == 9 else ()):
             self._ok(self.L.amrhydro_set_option(self.h, k, float(v)))
         self.hier = hier
         self.npatch = int(hier["level"].shape[0])
@@ -186,6 +188,9 @@ class AmrHydro:
 
     def reflux(self, coarse_level, slot=0):
         self._ok(self.L.amrhydro_reflux(self.h, coarse_level, slot))
+
+    def glm_damp(self, level, slot, factor):
+        self._ok(self.L.amrhydro_glm_damp(self.h, level, slot, factor))
 
     def copy_slot(self, level, src, dst):
         self._ok(self.L.amrhydro_copy_slot(self.h, level, src, dst))

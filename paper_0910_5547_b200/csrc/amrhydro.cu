@@ -29,6 +29,7 @@ struct amrhydro {
   double gamma = 1.4;
   int nv = 5, bits = 64;
   double theta = 1.5, rho_floor = 1e-30, e_floor = 1e-30;
+  double glm_ch = 1.0, glm_cr = 0.18;      // S17, S18 (nvars = 9)
   int kernel = 2, halo = 0;
   void *pool = nullptr;
   size_t pool_bytes = 0;
@@ -80,10 +81,12 @@ int fail(amrhydro *h, int code, const std::string &msg) {
 template <class F> int dispatch(amrhydro *h, F &&f) {
   if (h->bits == 64) {
     if (h->nv == 5) return f(double(0), std::integral_constant<int, 5>());
-    return f(double(0), std::integral_constant<int, 8>());
+    if (h->nv == 8) return f(double(0), std::integral_constant<int, 8>());
+    return f(double(0), std::integral_constant<int, 9>());
   }
   if (h->nv == 5) return f(float(0), std::integral_constant<int, 5>());
-  return f(float(0), std::integral_constant<int, 8>());
+  if (h->nv == 8) return f(float(0), std::integral_constant<int, 8>());
+  return f(float(0), std::integral_constant<int, 9>());
 }
 
 template <typename T> Params<T> make_params(const amrhydro *h) {
@@ -94,6 +97,7 @@ template <typename T> Params<T> make_params(const amrhydro *h) {
   P.theta = T(h->theta);
   P.rho_floor = T(h->rho_floor);
   P.e_floor = T(h->e_floor);
+  P.ch = T(h->glm_ch);
   return P;
 }
 template <typename T> Pool<T> make_pool(const amrhydro *h) { return Pool<T>{(T *)h->pool, h->maxp, h->nv}; }
@@ -147,7 +151,7 @@ void free_hierarchy(amrhydro *h) {
 extern "C" {
 
 amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) {
-  if (!(gamma > 1.0) || (nvars != 5 && nvars != 8) || patch_dim != NI || nghost != NG) return nullptr;
+  if (!(gamma > 1.0) || (nvars != 5 && nvars != 8 && nvars != 9) || patch_dim != NI || nghost != NG) return nullptr;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return nullptr;   // no CPU fallback
   amrhydro *h = new amrhydro;
@@ -193,6 +197,15 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
     case AMRHYDRO_OPT_HALO:
       if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "halo must be 0 or 1");
       h->halo = int(value);
+      return 0;
+    case AMRHYDRO_OPT_GLM_CH:
+      if (!(value > 0.0) || !std::isfinite(value)) return fail(h, AMRHYDRO_EINVAL, "c_h must be positive and finite");
+      h->glm_ch = value;
+      for (auto &sl : h->smax_slot) sl = -1;          // c_h enters the cached maxima
+      return 0;
+    case AMRHYDRO_OPT_GLM_CR:
+      if (!(value >= 0.0) || !std::isfinite(value)) return fail(h, AMRHYDRO_EINVAL, "c_r must be >= 0 and finite");
+      h->glm_cr = value;
       return 0;
     case AMRHYDRO_OPT_FUSE_CFL:
       if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "fuse_cfl must be 0, 1 or 2");
@@ -499,20 +512,26 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     const int n = h->lev_count[level], first = h->lev_first[level];
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
     smax_touch(h, level, sout);
+    if (NV == 9 && h->kernel != 0 && h->kernel != 2)
+      return fail(h, AMRHYDRO_EINVAL, "nvars = 9 runs on rk_stage kernels 0 and 2");
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
                                                                 T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
       LAUNCH_CHECK(h);
     } else if (h->kernel == 4) {
-      int r = launch_rk_stage_quad<T, NV>(h->tmap8, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
-      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_quad: ") + cudaGetErrorString((cudaError_t)r));
-      LAUNCH_CHECK(h);
+      if constexpr (NV != 9) {
+        int r = launch_rk_stage_quad<T, NV>(h->tmap8, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+        if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_quad: ") + cudaGetErrorString((cudaError_t)r));
+        LAUNCH_CHECK(h);
+      }
     } else if (h->kernel == 3) {
-      int r = launch_rk_stage_lite<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
-      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_lite: ") + cudaGetErrorString((cudaError_t)r));
-      LAUNCH_CHECK(h);
+      if constexpr (NV != 9) {
+        int r = launch_rk_stage_lite<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
+        if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_lite: ") + cudaGetErrorString((cudaError_t)r));
+        LAUNCH_CHECK(h);
+      }
     } else if (h->kernel == 2) {
       // the combination stage also reduces the max signal speed of what it writes (a1 fused into a6)
       const bool fuse = (h->fuse_cfl == 1 || (h->fuse_cfl == 2 && h->bits == 32)) && a != 0.0;
@@ -523,7 +542,7 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
       if (fuse) h->smax_slot[level] = sout;
-    } else {
+    } else if constexpr (NV != 9) {
       int r = launch_rk_stage_tile<T, NV>(make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                           make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_tile: ") + cudaGetErrorString((cudaError_t)r));
@@ -572,6 +591,21 @@ int amrhydro_reflux(amrhydro_t *h, int clev, int slot) {
   });
 }
 
+int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (h->nv != 9) return fail(h, AMRHYDRO_EINVAL, "glm_damp needs the 9-variable system");
+  if (!std::isfinite(factor)) return fail(h, AMRHYDRO_EINVAL, "factor must be finite");
+  return dispatch(h, [&](auto t, auto nv) {          // psi does not enter the signal speeds: cached maxima stay valid
+    using T = decltype(t);
+    k_scale_var<T><<<h->lev_count[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level], 8, T(factor));
+    LAUNCH_CHECK(h);
+    (void)nv;
+    return 0;
+  });
+}
+
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {
   if (int r = check_ready(h)) return r;
   if (int r = check_level(h, level)) return r;
@@ -596,6 +630,8 @@ static int advance_level(amrhydro_t *h, int lev, double dt, double a1, double a2
   if ((r = amrhydro_rk_stage(h, lev, 0, 0, 1, 0.0, 1.0, dt, w))) return r;      // U1 = Un + dt L(Un)
   if ((r = amrhydro_fill_ghosts(h, lev, 1, 2, 0, a2))) return r;
   if ((r = amrhydro_rk_stage(h, lev, 1, 0, 0, 0.5, 0.5, dt, w))) return r;      // Un+1 = (Un + U1 + dt L(U1))/2
+  if (h->nv == 9 && h->glm_cr > 0.0 &&                                           // S18
+      (r = amrhydro_glm_damp(h, lev, 0, std::exp(-dt * h->glm_ch / h->glm_cr)))) return r;
   if (kids) {
     if ((r = amrhydro_fill_ghosts(h, lev, 0, 2, 0, a2))) return r;
     if ((r = advance_level(h, lev + 1, 0.5 * dt, 0.0, 0.5))) return r;

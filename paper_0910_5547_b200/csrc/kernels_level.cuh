@@ -29,6 +29,15 @@ __global__ void __launch_bounds__(256) k_unpack(Pool<T> pool, int slot, int firs
     dst[c] = src[cell<T>(k + NG, j + NG, i + NG)];
   }
 }
+// interior cells of one variable times a factor (S18: psi <- psi exp(-dt c_h / c_r))
+template <typename T>
+__global__ void __launch_bounds__(256) k_scale_var(Pool<T> pool, int slot, int first, int v, T factor) {
+  T *u = pool.patch(slot, first + blockIdx.x) + size_t(v) * Layout<T>::VS;
+  for (int c = threadIdx.x; c < NI * NI * NI; c += 256) {
+    const int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
+    u[cell<T>(k + NG, j + NG, i + NG)] *= factor;
+  }
+}
 // padded box of one patch as doubles [var][20][20][20] (tests)
 template <typename T>
 __global__ void k_unpack_padded(Pool<T> pool, int slot, int p, double *__restrict__ out) {

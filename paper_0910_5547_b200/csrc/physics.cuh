@@ -17,6 +17,7 @@ template <typename T> struct Params {
   T gamma, gm1, gg1;   // gamma, gamma-1, gamma*(gamma-1)
   T theta;             // Eq. 9-10 (S1)
   T rho_floor, e_floor;
+  T ch;                // c_h of Eq. 15 (9-variable GLM-MHD only; S17)
 };
 
 __device__ __forceinline__ float tsqrt(float x) { return sqrtf(x); }
@@ -61,10 +62,11 @@ __device__ __forceinline__ void cons_to_prim(const T (&U)[NV], T (&W)[NV], const
   T ir = trcp(rho);
   T vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
   T et = U[4];
-  if (NV == 8) {
-    et -= T(0.5) * (U[5] * U[5] + U[6] * U[6] + U[7] * U[7]);
+  if (NV >= 8) {
+    et -= T(0.5) * (U[5 % NV] * U[5 % NV] + U[6 % NV] * U[6 % NV] + U[7 % NV] * U[7 % NV]);
     W[5 % NV] = U[5 % NV]; W[6 % NV] = U[6 % NV]; W[7 % NV] = U[7 % NV];
   }
+  if (NV == 9) W[8 % NV] = U[8 % NV];                             // psi (Eq. 14)
   T e = et * ir - T(0.5) * (vx * vx + vy * vy + vz * vz);
   if (!(e >= P.e_floor)) { e = P.e_floor; ++hits; }
   W[0] = rho; W[1] = e; W[2] = vx; W[3] = vy; W[4] = vz;
@@ -107,6 +109,11 @@ __device__ __forceinline__ void state_flux(const T (&W)[NV], const Params<T> &P,
     F[4] = (E + pt) * vd - Bd * Bv;                               // Eq. 15 energy row
     F[5 % NV] = vd * Bx - Bd * W[2]; F[6 % NV] = vd * By - Bd * W[3]; F[7 % NV] = vd * Bz - Bd * W[4];
     F[(5 + D) % NV] = T(0);                                       // psi == 0 (S3')
+    if (NV == 9) {                                                // Eq. 15: F^d(B_d) = psi, F^d(psi) = c_h^2 B_d
+      U[8 % NV] = W[8 % NV];
+      F[(5 + D) % NV] = W[8 % NV];
+      F[8 % NV] = P.ch * P.ch * Bd;
+    }
     const T ir = trcp(rho);                                       // S3: fast magnetosonic speed along D
     const T a2 = P.gg1 * e, b2 = B2 * ir, bd2 = Bd * Bd * ir;
     const T s = a2 + b2;
@@ -122,7 +129,8 @@ __device__ __forceinline__ void riemann_flux(const T (&WL)[NV], const T (&WR)[NV
   T UL[NV], UR[NV], FL[NV], FR[NV], sl, sr;
   state_flux<T, NV, D>(WL, P, UL, FL, sl);
   state_flux<T, NV, D>(WR, P, UR, FR, sr);
-  const T lam = tmax(sl, sr);
+  T lam = tmax(sl, sr);
+  if (NV == 9) lam = tmax(lam, P.ch);                             // S17
 #pragma unroll
   for (int v = 0; v < NV; ++v) F[v] = T(0.5) * ((FL[v] + FR[v]) - lam * (UR[v] - UL[v]));
 }
@@ -144,6 +152,7 @@ __device__ __forceinline__ T max_signal_speed(const T (&W)[NV], const Params<T> 
       const T disc = tmax(s * s - T(4) * a2 * bd2, T(0));
       best = tmax(best, tabs(W[2 + d]) + tsqrt(T(0.5) * (s + tsqrt(disc))));
     }
+    if (NV == 9) best = tmax(best, P.ch);                         // S17: c_h bounds the time step too
     return best;
   }
 }

@@ -89,10 +89,11 @@ __device__ __forceinline__ void prim(const T (&U)[NV], T (&W)[NV], const Params<
   const T ir = frcp(rho);
   const T vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
   T et = U[4];
-  if (NV == 8) {
+  if (NV >= 8) {
     et = fma(T(-0.5), fma(U[7 % NV], U[7 % NV], fma(U[6 % NV], U[6 % NV], U[5 % NV] * U[5 % NV])), et);
     W[5 % NV] = U[5 % NV]; W[6 % NV] = U[6 % NV]; W[7 % NV] = U[7 % NV];
   }
+  if (NV == 9) W[8 % NV] = U[8 % NV];                               // psi (Eq. 14)
   T e = fma(T(-0.5), fma(vz, vz, fma(vy, vy, vx * vx)), et * ir);
   if (hiw(e) <= hiw(P.e_floor)) {
     if (below(e, P.e_floor)) { e = P.e_floor; ++hits; }
@@ -151,9 +152,11 @@ __device__ __forceinline__ void face_flux(const T (&L)[5], const T (&R)[5], cons
   G[4] = fma(A, hr, fma(B, hl, fma(pr, vdr, pl * vdl)));
 }
 
-// ideal MHD, Eq. 15 with G3 and psi == 0 (S3'); fast magnetosonic speed along D (S3)
-template <typename T, int D>
-__device__ __forceinline__ void mhd_state(const T (&W)[8], const Params<T> &P, T (&U)[8], T (&F)[8], T &speed) {
+// MHD, Eq. 15 with G3: NV = 8 ideal (psi == 0, S3'), NV = 9 GLM (F^d(B_d) = psi, F^d(psi) = c_h^2 B_d);
+// fast magnetosonic speed along D (S3)
+template <typename T, int D, int NV>
+__device__ __forceinline__ void mhd_state(const T (&W)[NV], const Params<T> &P, T (&U)[NV], T (&F)[NV], T &speed) {
+  static_assert(NV == 8 || NV == 9, "MHD variable sets");
   const T rho = W[0], e = W[1], vd = W[2 + D];
   const T re = rho * e, p = P.gm1 * re, m = rho * vd;
   const T q2 = fma(W[4], W[4], fma(W[3], W[3], W[2] * W[2]));
@@ -169,6 +172,11 @@ __device__ __forceinline__ void mhd_state(const T (&W)[8], const Params<T> &P, T
   F[4] = fma(E + pt, vd, -(Bd * Bv));
   F[5] = fma(vd, Bx, -(Bd * W[2])); F[6] = fma(vd, By, -(Bd * W[3])); F[7] = fma(vd, Bz, -(Bd * W[4]));
   F[5 + D] = T(0);
+  if (NV == 9) {
+    U[8 % NV] = W[8 % NV];
+    F[5 + D] = W[8 % NV];
+    F[8 % NV] = P.ch * P.ch * Bd;
+  }
   const T ir = frcp(rho);
   const T a2 = P.gg1 * e, s = fma(B2, ir, a2), bd2 = Bd * Bd * ir;
   const T disc = fma(s, s, T(-4) * a2 * bd2);
@@ -176,14 +184,15 @@ __device__ __forceinline__ void mhd_state(const T (&W)[8], const Params<T> &P, T
   const T sq = disc > T(1e-30) * s * s ? fsqrt(disc) : T(0);
   speed = tabs(vd) + fsqrt(T(0.5) * (s + sq));
 }
-template <typename T, int D>
-__device__ __forceinline__ void face_flux(const T (&L)[8], const T (&R)[8], const Params<T> &P, T (&G)[8]) {
-  T UL[8], UR[8], FL[8], FR[8], sl, sr;
-  mhd_state<T, D>(L, P, UL, FL, sl);
-  mhd_state<T, D>(R, P, UR, FR, sr);
-  const T lam = sl > sr ? sl : sr;
+template <typename T, int D, int NV>
+__device__ __forceinline__ void face_flux(const T (&L)[NV], const T (&R)[NV], const Params<T> &P, T (&G)[NV]) {
+  T UL[NV], UR[NV], FL[NV], FR[NV], sl, sr;
+  mhd_state<T, D, NV>(L, P, UL, FL, sl);
+  mhd_state<T, D, NV>(R, P, UR, FR, sr);
+  T lam = sl > sr ? sl : sr;
+  if (NV == 9) lam = lam > P.ch ? lam : P.ch;                       // S17
 #pragma unroll
-  for (int v = 0; v < 8; ++v) G[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
+  for (int v = 0; v < NV; ++v) G[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
 }
 
 // fp32: the same value from the 3-input min/max of sm_100 (FMNMX3): with x = 2 theta dm, y = 2 theta dp,
@@ -368,7 +377,7 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
 }  // namespace mk
 
 template <typename T, int NV, bool BASE>
-__global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : AMR_MINB32))
+__global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? AMR_MINB32 : 2)))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
                  const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out) {

@@ -24,7 +24,7 @@ def gpu():
 def make_pair(gpu, h, gamma, nv, dtype="f64", ncpu=8, **kw):
     import oracle
     g = gpu.AmrHydro(h, gamma, nv, dtype=dtype, **kw)
-    o = oracle.Oracle(h, gamma, nv, threads=ncpu, theta=kw.get("theta", 1.5))
+    o = oracle.Oracle(h, gamma, nv, threads=ncpu, theta=kw.get("theta", 1.5), ch=kw.get("ch", 1.0), cr=kw.get("cr", 0.18))
     return g, o
 
 
@@ -42,8 +42,9 @@ def rand_state(h, nv, seed, gamma=1.4):
     shp = (n, 16, 16, 16)
     rho = rng.uniform(0.5, 1.5, shp); p = rng.uniform(0.5, 1.5, shp)
     v = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)]
-    B = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)] if nv == 8 else None
-    return np.moveaxis(wl.cons_from_prim(rho, p, v, gamma, B=B), 0, 1).copy()
+    B = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)] if nv >= 8 else None
+    psi = rng.uniform(-0.2, 0.2, shp) if nv == 9 else None
+    return np.moveaxis(wl.cons_from_prim(rho, p, v, gamma, B=B, psi=psi), 0, 1).copy()
 
 
 # ------------------------------------------------------------------ a1: CFL reduction
@@ -154,12 +155,14 @@ def test_fill_ghosts_prolongation_matches_oracle(gpu, kind, alpha):
 
 
 # ------------------------------------------------------------------ a3-a6: one stage
-@pytest.mark.parametrize("nv", [5, 8])
+@pytest.mark.parametrize("nv", [5, 8, 9])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("kernel,halo", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1), (4, 0), (4, 1)])
 def test_rk_stage_matches_oracle(gpu, nv, dtype, kernel, halo):
+    if nv == 9 and kernel not in (0, 2):
+        pytest.skip("the 9-variable system runs on the reference and the default stage kernel")
     h = wl.uniform_hierarchy(2, periodic=True)
-    g, o = make_pair(gpu, h, 5.0 / 3.0, nv, dtype, kernel=kernel, halo=halo)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, nv, dtype, kernel=kernel, halo=halo, ch=1.7)
     upload_both(g, o, rand_state(h, nv, 6, 5.0 / 3.0), dtype)
     dt = 0.3 * o.cfl_dt(0, 0, 1.0)
     for x in (g, o):
@@ -299,6 +302,49 @@ def test_config5_stress_reduced(gpu, dtype):
     upload_both(g, o, wl.split_global(h, wl.stress_global(64)), dtype)
     G, O = run_both(g, o, 3, 0.3)
     assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
+
+
+# ------------------------------------------------------------------ 9-variable GLM-MHD (NEXT-1)
+def test_glm_cfl_sees_ch_and_damp_matches_oracle(gpu):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 9, ch=25.0)
+    upload_both(g, o, rand_state(h, 9, 31, 5.0 / 3.0), "f64")
+    dt = g.cfl_dt(0, 0, 0.3)
+    assert dt == 0.3 * (1.0 / 32) / 25.0 and abs(dt - o.cfl_dt(0, 0, 0.3)) <= 1e-15 * dt     # S17
+    g.set_option(gpu.OPT_GLM_CH, 0.01)                                 # the cached maximum must not survive
+    o2 = make_pair(gpu, h, 5.0 / 3.0, 9, ch=0.01)[1]
+    o2.upload(0, o.download(0))
+    assert abs(g.cfl_dt(0, 0, 0.3) - o2.cfl_dt(0, 0, 0.3)) <= 1e-14 * dt * 2500
+    for x in (g, o):
+        x.glm_damp(0, 0, 0.625)
+    assert np.array_equal(g.download(0), o.download(0))
+    g5 = gpu.AmrHydro(h, 1.4, 5)
+    with pytest.raises(gpu.AmrHydroError):
+        g5.glm_damp(0, 0, 0.5)
+
+
+@pytest.mark.parametrize("halo,dtype", [(0, "f64"), (1, "f64"), (1, "f32")])
+def test_glm_mhd_turbulence_with_damping(gpu, halo, dtype):
+    h = wl.uniform_hierarchy(2, periodic=True)
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 9, dtype, halo=halo, ch=2.5, cr=0.18)
+    G8 = wl.mhd_turbulence_global(32)
+    rng = np.random.default_rng(33)
+    G8[5:8] += 0.05 * rng.standard_normal(G8[5:8].shape)               # not solenoidal any more: psi gets to work
+    G9 = np.concatenate([G8, np.zeros_like(G8[:1])])
+    U = upload_both(g, o, wl.split_global(h, G9), dtype)
+    G, O = run_both(g, o, 10, 0.3)
+    assert np.abs(O[:, 8]).max() > 1e-3 and np.isfinite(G).all()
+    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
+
+
+def test_glm_amr_two_level(gpu):
+    h = amr_hier("slab")
+    g, o = make_pair(gpu, h, 5.0 / 3.0, 9, ch=2.0, cr=0.18)
+    upload_both(g, o, rand_state(h, 9, 34, 5.0 / 3.0), "f64")
+    for x in (g, o):
+        x.restrict(1)
+    G, O = run_both(g, o, 2, 0.3)
+    assert norm_err(G, O).max() <= 1e-12
 
 
 def test_amr_mhd_two_level(gpu):

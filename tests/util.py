@@ -85,7 +85,7 @@ def norm_err(a, b, vector=False):
     of every component alike."""
     groups = [[v] for v in range(b.shape[1])]
     if vector:
-        groups = [[0], [1, 2, 3], [4]] + ([[5, 6, 7]] if b.shape[1] == 8 else [])
+        groups = [[0], [1, 2, 3], [4]] + ([[5, 6, 7]] if b.shape[1] >= 8 else []) + ([[8]] if b.shape[1] == 9 else [])
     out = []
     for grp in groups:
         s = max(np.abs(b[:, v]).max() for v in grp)
