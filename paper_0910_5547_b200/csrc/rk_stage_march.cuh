@@ -488,7 +488,6 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
       if (c > NG) {
         const T *ui = raw + ((c - 1) % S::NSLOT) * RAWP;     // raw U of cell c-1 is still in the ring
         T *o = out + (c - 1) * PLANE;
-#pragma unroll
         T un[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
