@@ -1,0 +1,111 @@
+"""GPU edge cases of the C ABI against the oracle: error behaviour, empty ranges, non-cubic and
+one-patch-thick base grids, a level with a single patch, AMR in fp32 and with direct sibling halos
+(the launch configuration bench.py uses for config 3)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_0910_5547_b200 import workloads as wl  # noqa: E402
+from util import norm_err  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_0910_5547_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def rand_state(h, nv, seed, gamma=1.4):
+    rng = np.random.default_rng(seed)
+    shp = (len(h["level"]), 16, 16, 16)
+    rho = rng.uniform(0.5, 1.5, shp); p = rng.uniform(0.5, 1.5, shp)
+    v = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)]
+    B = [rng.uniform(-0.5, 0.5, shp) for _ in range(3)] if nv >= 8 else None
+    return np.moveaxis(wl.cons_from_prim(rho, p, v, gamma, B=B), 0, 1).copy()
+
+
+def pair(gpu, h, gamma, nv, dtype="f64", **kw):
+    import oracle
+    return gpu.AmrHydro(h, gamma, nv, dtype=dtype, **kw), oracle.Oracle(h, gamma, nv, threads=8)
+
+
+def test_errors_are_reported_and_do_not_poison_the_handle(gpu):
+    h = wl.uniform_hierarchy(1, periodic=True)
+    g = gpu.AmrHydro(h, 1.4, 5)
+    U = rand_state(h, 5, 1)
+    g.upload(0, U)
+    bad = [lambda: g.rk_stage(0, 0, 0, 0, 0.0, 1.0, 1e-3),        # slot_out == slot_in
+           lambda: g.rk_stage(0, 0, 0, 7, 0.0, 1.0, 1e-3),        # slot out of range
+           lambda: g.rk_stage(3, 0, 0, 1, 0.0, 1.0, 1e-3),        # level out of range
+           lambda: g.fill_ghosts(-1, 0),
+           lambda: g.cfl_dt(0, 9, 0.3),
+           lambda: g.restrict(1),                                  # no fine level
+           lambda: g.set_option(gpu.OPT_THETA, 2.5),
+           lambda: g.set_option(gpu.OPT_KERNEL, 11),
+           lambda: g.set_option(99, 1.0),
+           lambda: g.upload(0, np.concatenate([U, U]))]            # more patches than the hierarchy holds
+    for f in bad:
+        with pytest.raises(gpu.AmrHydroError):
+            f()
+    g.fill_ghosts(0, 0)
+    g.rk_stage(0, 0, 0, 1, 0.0, 1.0, 1e-3)                         # still usable
+    assert np.isfinite(g.download(1)).all()
+    g.upload(0, U[:0])                                             # empty ranges are no-ops
+    assert g.download(0, 0, 0).shape == (0, 5, 16, 16, 16)
+    assert np.array_equal(g.download(0), U)
+    assert g.L.amrhydro_create(1.0, 5, 16, 2) is None and g.L.amrhydro_create(1.4, 7, 16, 2) is None
+    assert g.L.amrhydro_create(1.4, 5, 32, 2) is None and g.L.amrhydro_create(1.4, 5, 16, 3) is None
+
+
+@pytest.mark.parametrize("nb,periodic", [((3, 1, 2), True), ((1, 1, 1), False), ((1, 4, 1), False)])
+@pytest.mark.parametrize("halo", [0, 1])
+def test_non_cubic_and_one_patch_thick_grids(gpu, nb, periodic, halo):
+    h = wl.uniform_hierarchy(nb, periodic=periodic)
+    g, o = pair(gpu, h, 1.4, 5, halo=halo)
+    U = rand_state(h, 5, 2)
+    g.upload(0, U); o.upload(0, U)
+    for _ in range(3):
+        dt = o.advance(0.3)
+        assert abs(g.advance(0.3) - dt) <= 1e-13 * dt
+    assert norm_err(g.download(0), o.download(0)).max() <= 1e-12
+
+
+def single_child_hierarchy():
+    return wl.build_hierarchy((2, 2, 2), [[(1, 2, 1)]], (0,) * 6)     # one fine patch = one octant of one coarse patch
+
+
+@pytest.mark.parametrize("halo", [0, 1])
+def test_level_with_a_single_patch(gpu, halo):
+    h = single_child_hierarchy()
+    assert int((np.asarray(h["level"]) == 1).sum()) == 1
+    g, o = pair(gpu, h, 1.4, 5, halo=halo)
+    U = rand_state(h, 5, 3)
+    g.upload(0, U); o.upload(0, U)
+    for x in (g, o):
+        x.restrict(1)
+    for _ in range(2):
+        dt = o.advance(0.3)
+        g.advance(0.3, dt)
+    assert norm_err(g.download(0), o.download(0)).max() <= 1e-12
+
+
+@pytest.mark.parametrize("dtype,halo", [("f64", 1), ("f32", 0), ("f32", 1)])
+def test_sedov_amr_fp32_and_direct_halos(gpu, dtype, halo):
+    """config 3 reduced (32^3 base + 3 levels), in the bench's launch configuration (halo = 1) and in fp32."""
+    h = wl.ball_hierarchy(2, 4, bc=(1,) * 6)
+    g, o = pair(gpu, h, 1.4, 5, dtype, halo=halo)
+    U = wl.sedov_hierarchy_state(h)
+    if dtype == "f32":
+        U = U.astype(np.float32).astype(np.float64)
+    g.upload(0, U); o.upload(0, U)
+    for _ in range(2):
+        dt = o.advance(0.3)
+        g.advance(0.3, dt)
+    G, O = g.download(0).astype(np.float64), o.download(0)
+    assert np.isfinite(G).all()
+    assert norm_err(G, O, vector=(dtype == "f32")).max() <= (1e-12 if dtype == "f64" else 1e-5)
