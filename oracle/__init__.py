@@ -68,6 +68,8 @@ def lib():
         L.orc_face.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int] + [dp] * 7
         L.orc_prim.argtypes = [C.c_int, C.c_double, dp, dp]
         L.orc_flux.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, dp, dp]
+        L.orc_refine_indicator.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+        L.orc_prolong_interior.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.orc_set_glm.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orc_set_glm.restype = None
         L.orc_glm_damp.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double]
@@ -213,6 +215,17 @@ class Oracle:
     def reflux(self, coarse_level, slot=0):
         if lib().orc_reflux(self.h, coarse_level, slot):
             raise ValueError("reflux: improper nesting")
+
+    def refine_indicator(self, level, slot=0):
+        """S20: max of |grad rho|/rho over each octant of each patch of the level -> [npatch_level][8]."""
+        n = int((np.asarray(self.hier["level"]) == level).sum())
+        out = np.zeros((n, 8))
+        lib().orc_refine_indicator(self.h, level, slot, _dp(out))
+        return out
+
+    def prolong_interior(self, patch, slot=0, parent_slot=0):
+        if lib().orc_prolong_interior(self.h, patch, slot, parent_slot):
+            raise ValueError("prolong_interior: bad patch")
 
     def glm_damp(self, level, slot, factor):
         lib().orc_glm_damp(self.h, level, slot, factor)

@@ -329,6 +329,56 @@ template <class T> struct Hier {
     });
   }
 
+  // ---- regrid steps on either side of the hot path (readings S20-S21 of DESIGN.md)
+  // S20: refinement indicator of BASELINE.json config 3, |grad rho| / rho with centred differences over the
+  // ghost-filled padded box, reduced to its maximum over each 8^3 octant of every patch of the level (the
+  // footprint of one would-be child patch).  out[n*8 + o], n = index in the level, o = octant (x bit 0).
+  void refine_indicator(int lev, int slot, double *out) {
+    const auto &lp = lev_patches[lev];
+    const double dx = dx0 / double(1 << lev);
+    for (size_t n = 0; n < lp.size(); ++n) {
+      const T *rho = P(slot, lp[n]);
+      for (int o = 0; o < 8; ++o) out[n * 8 + o] = 0.0;
+      for (int k = NG; k < NG + NI; ++k)
+        for (int j = NG; j < NG + NI; ++j)
+          for (int i = NG; i < NG + NI; ++i) {
+            double gx = (double(rho[cidx(k, j, i + 1)]) - double(rho[cidx(k, j, i - 1)])) / (2.0 * dx);
+            double gy = (double(rho[cidx(k, j + 1, i)]) - double(rho[cidx(k, j - 1, i)])) / (2.0 * dx);
+            double gz = (double(rho[cidx(k + 1, j, i)]) - double(rho[cidx(k - 1, j, i)])) / (2.0 * dx);
+            double g = std::sqrt(gx * gx + gy * gy + gz * gz) / double(rho[cidx(k, j, i)]);
+            int o = ((i - NG) >> 3) | (((j - NG) >> 3) << 1) | (((k - NG) >> 3) << 2);
+            if (!(g <= out[n * 8 + o])) out[n * 8 + o] = g;   // NaN propagates
+          }
+    }
+  }
+  // S21: interior of a (new) fine patch from its parent's padded box with the operator of S6
+  // (conservative limited-linear; the 8 children of a coarse cell average to it).
+  void prolong_interior(int p, int slot, int pslot) {
+    int Q = parent[p];
+    T *U = P(slot, p);
+    const T *C = P(pslot, Q);
+    for (int k = NG; k < NG + NI; ++k)
+      for (int j = NG; j < NG + NI; ++j)
+        for (int i = NG; i < NG + NI; ++i) {
+          int pad[3] = {i, j, k}, pc[3];
+          T sg[3];
+          for (int d = 0; d < 3; ++d) {
+            int g = origin[size_t(p) * 3 + d] + pad[d] - NG;
+            int gc = g / 2;                                              // g >= 0 on interior cells
+            sg[d] = (g - 2 * gc == 0) ? T(-0.25) : T(0.25);
+            pc[d] = gc - origin[size_t(Q) * 3 + d] + NG;
+          }
+          int c0 = cidx(pc[2], pc[1], pc[0]);
+          const int st[3] = {1, NP, NP * NP};
+          for (int v = 0; v < nv; ++v) {
+            const T *c = C + size_t(v) * NC;
+            T uc = c[c0], val = uc;
+            for (int d = 0; d < 3; ++d) val = val + sg[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
+            U[size_t(v) * NC + cidx(k, j, i)] = val;
+          }
+        }
+  }
+
   // ---- O1-O4: one RK stage on every patch of a level.
   // U_out = a U_base + b (U_in + dt L(U_in)) on interior cells; Eq. 7-8 PAPER.md:79-98.
   // w != 0 accumulates w*dt*F on coarse-fine faces (reading S10).
@@ -664,6 +714,12 @@ int orc_rk_stage(void *h, int lev, int sin, int sbase, int sout, double a, doubl
 }
 int orc_restrict(void *h, int flev, int fslot, int cslot) { DISPATCH(h, H.restrict_level(flev, fslot, cslot)); return 0; }
 int orc_reflux(void *h, int clev, int slot) { int r = 0; DISPATCH(h, r = H.reflux(clev, slot)); return r; }
+int orc_refine_indicator(void *h, int lev, int slot, double *out) { DISPATCH(h, H.refine_indicator(lev, slot, out)); return 0; }
+int orc_prolong_interior(void *h, int p, int slot, int pslot) {
+  int r = 0;
+  DISPATCH(h, { if (p < 0 || p >= H.np || H.level[p] == 0) r = -1; else H.prolong_interior(p, slot, pslot); });
+  return r;
+}
 int orc_copy_slot(void *h, int lev, int src, int dst) { DISPATCH(h, H.copy_slot(lev, src, dst)); return 0; }
 // one coarse step of the whole hierarchy (O5 when nlev == 1); returns dt0 used
 int orc_advance(void *h, double cfl, double dt_fixed, double *dt_out) {
