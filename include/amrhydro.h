@@ -159,6 +159,18 @@ int amrhydro_reflux(amrhydro_t *h, int coarse_level, int slot);
 
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src_slot, int dst_slot);
 
+/* Regrid steps on either side of the hot path (PAPER.md:43-45 leaves regridding to the
+ * host code; the table itself is rebuilt by the caller and handed to amrhydro_set_hierarchy).
+ * refine_indicator (S20): for every patch of the level and each of its eight 8^3 octants (x = bit 0, y = bit 1,
+ * z = bit 2) the maximum of |grad rho| / rho, centred differences over the padded box (ghosts must be
+ * filled); host_octmax[count_of_level][8] doubles; synchronises.  Thresholding (BASELINE config 3: above
+ * 0.1 of the level maximum) is the caller's.  A NaN anywhere in an octant gives NaN for that octant.
+ * prolong_interior (S21): the 16^3 interior of fine patch `patch` in `slot` from the padded box of its
+ * parent in `parent_slot` (conservative limited-linear, the operator of S6); the parent's ghosts must be
+ * filled.  AMRHYDRO_EINVAL for a level-0 patch. */
+int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_octmax);
+int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slot);
+
 /* nvars = 9 only (AMRHYDRO_EINVAL otherwise): psi <- factor * psi on the interior cells of one level,
  * the damping of the mixed GLM system of Dedner et al. 2002 adopted at PAPER.md:292 (S18);
  * amrhydro_advance calls it after every step of a level with factor = exp(-dt_l c_h / c_r). */

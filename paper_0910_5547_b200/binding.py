@@ -21,7 +21,8 @@ EXPORTS = [
     "amrhydro_get_counter", "amrhydro_pool_bytes", "amrhydro_bind_pool", "amrhydro_set_hierarchy",
     "amrhydro_upload", "amrhydro_download", "amrhydro_download_padded", "amrhydro_download_registers",
     "amrhydro_cfl_dt", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
-    "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
+    "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_refine_indicator",
+    "amrhydro_prolong_interior", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
 ]
 
 
@@ -65,6 +66,8 @@ def load_library():
     L.amrhydro_reflux.argtypes = [vp, i, i]
     L.amrhydro_copy_slot.argtypes = [vp, i, i, i]
     L.amrhydro_glm_damp.argtypes = [vp, i, i, d]
+    L.amrhydro_refine_indicator.argtypes = [vp, i, i, dp]
+    L.amrhydro_prolong_interior.argtypes = [vp, i, i, i]
     L.amrhydro_advance.argtypes = [vp, d, d, dp]
     L.amrhydro_advance_host.argtypes = [vp, d, d, i, vp, vp, dp]
     L.amrhydro_sync.argtypes = [vp]
@@ -188,6 +191,15 @@ class AmrHydro:
 
     def reflux(self, coarse_level, slot=0):
         self._ok(self.L.amrhydro_reflux(self.h, coarse_level, slot))
+
+    def refine_indicator(self, level, slot=0):
+        n = int((np.asarray(self.hier["level"]) == level).sum())
+        out = np.zeros((n, 8))
+        self._ok(self.L.amrhydro_refine_indicator(self.h, level, slot, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def prolong_interior(self, patch, slot=0, parent_slot=0):
+        self._ok(self.L.amrhydro_prolong_interior(self.h, patch, slot, parent_slot))
 
     def glm_damp(self, level, slot, factor):
         self._ok(self.L.amrhydro_glm_damp(self.h, level, slot, factor))

@@ -606,6 +606,42 @@ int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor) {
   });
 }
 
+int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_octmax) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!host_octmax) return fail(h, AMRHYDRO_EINVAL, "host_octmax is null");
+  const int n = h->lev_count[level];
+  const size_t bytes = size_t(n) * 8 * sizeof(double);
+  if (int r = ensure_stage(h, bytes)) return r;
+  const double inv2dx = 0.5 / (h->dx0 / double(1 << level));
+  int r = dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    k_refine_indicator<T><<<n, 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level], inv2dx, (double *)h->d_stage);
+    LAUNCH_CHECK(h);
+    (void)nv;
+    return 0;
+  });
+  if (r) return r;
+  CUDA_TRY(h, cudaMemcpyAsync(host_octmax, h->d_stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slot) {
+  if (int r = check_ready(h)) return r;
+  if (check_slot(h, slot) || check_slot(h, parent_slot)) return AMRHYDRO_EINVAL;
+  if (patch < 0 || patch >= h->np || h->tbl[patch].level == 0) return fail(h, AMRHYDRO_EINVAL, "patch has no parent");
+  smax_touch(h, h->tbl[patch].level, slot);
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    k_prolong_interior<T, NV><<<NI, 256, 0, h->stream>>>(make_pool<T>(h), slot, parent_slot, patch, h->d_desc);
+    LAUNCH_CHECK(h);
+    return 0;
+  });
+}
+
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {
   if (int r = check_ready(h)) return r;
   if (int r = check_level(h, level)) return r;

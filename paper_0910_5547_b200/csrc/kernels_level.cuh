@@ -208,6 +208,79 @@ __global__ void __launch_bounds__(256) k_fill_outflow(Pool<T> pool, int slot, in
   }
 }
 
+// ------------------------------------------------------------------ regrid steps (NEXT-3; S20, S21)
+// S20: max over each 8^3 octant of |grad rho| / rho, centred differences over the ghost-filled box.
+// One block per patch; thread (j, i) walks k; octant maxima by warp shuffles + shared memory.
+// Always in double (it feeds a host-side threshold).  out[(patch_local)*8 + octant].
+template <typename T>
+__global__ void __launch_bounds__(256) k_refine_indicator(Pool<T> pool, int slot, int first, double inv2dx,
+                                                          double *__restrict__ out) {
+  const T *rho = pool.patch(slot, first + blockIdx.x);
+  const int i = threadIdx.x & 15, j = threadIdx.x >> 4;
+  constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE;
+  double best[2] = {0.0, 0.0};
+  bool bad = false;
+#pragma unroll 4
+  for (int k = 0; k < NI; ++k) {
+    const int c = cell<T>(k + NG, j + NG, i + NG);
+    const double gx = (double(rho[c + 1]) - double(rho[c - 1])) * inv2dx;
+    const double gy = (double(rho[c + PX]) - double(rho[c - PX])) * inv2dx;
+    const double gz = (double(rho[c + PLANE]) - double(rho[c - PLANE])) * inv2dx;
+    const double g = sqrt(gx * gx + gy * gy + gz * gz) / double(rho[c]);
+    bad |= !(g - g == 0.0);
+    best[k >> 3] = fmax(best[k >> 3], g);
+  }
+  // octant maxima on the bit pattern of a non-negative double (monotone as an unsigned integer; a NaN
+  // pattern is larger than every finite one, so it survives the maximum)
+  __shared__ unsigned long long smax[8];
+  if (threadIdx.x < 8) smax[threadIdx.x] = 0ull;
+  __syncthreads();
+#pragma unroll
+  for (int kz = 0; kz < 2; ++kz) {
+    const double b = bad ? __longlong_as_double(0x7ff8000000000000LL) : best[kz];
+    atomicMax(&smax[(i >> 3) | ((j >> 3) << 1) | (kz << 2)], (unsigned long long)__double_as_longlong(b));
+  }
+  __syncthreads();
+  if (threadIdx.x < 8) out[size_t(blockIdx.x) * 8 + threadIdx.x] = __longlong_as_double((long long)smax[threadIdx.x]);
+}
+
+// S21: all interior cells of fine patch p from its parent's padded box (operator of S6, one slot).
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_prolong_interior(Pool<T> pool, int slot, int pslot, int p,
+                                                          const Desc *__restrict__ desc) {
+  const Desc &D = desc[p];
+  const int Q = D.parent;
+  T *U = pool.patch(slot, p);
+  const T *C = pool.patch(pslot, Q);
+  const int ox = D.origin[0] - 2 * desc[Q].origin[0], oy = D.origin[1] - 2 * desc[Q].origin[1],
+            oz = D.origin[2] - 2 * desc[Q].origin[2];           // 0 or 16: the octant
+  const int k = blockIdx.x;                                      // one interior plane per block
+  const int i = threadIdx.x & 15, j = threadIdx.x >> 4;
+  const int g[3] = {ox + i, oy + j, oz + k};                     // fine index relative to the parent's corner
+  int c0;
+  T sg[3];
+  {
+    int pc[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      pc[d] = (g[d] >> 1) + NG;
+      sg[d] = (g[d] & 1) ? T(0.25) : T(-0.25);
+    }
+    c0 = cell<T>(pc[2], pc[1], pc[0]);
+  }
+  const int st[3] = {1, Layout<T>::PX, Layout<T>::PLANE};
+  const int me = cell<T>(k + NG, j + NG, i + NG);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const T *c = C + size_t(v) * Layout<T>::VS;
+    const T uc = c[c0];
+    T val = uc;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) val = val + sg[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
+    U[size_t(v) * Layout<T>::VS + me] = val;
+  }
+}
+
 // ------------------------------------------------------------------ a7: restriction (S8)
 // One block per fine patch; each thread produces coarse cells (pairwise tree sum, so that a
 // uniform state is restricted bitwise).
