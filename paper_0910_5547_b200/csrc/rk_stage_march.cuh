@@ -153,30 +153,24 @@ __device__ __forceinline__ void face_flux(const T (&L)[5], const T (&R)[5], cons
 }
 
 // MHD, Eq. 15 with G3: NV = 8 ideal (psi == 0, S3'), NV = 9 GLM (F^d(B_d) = psi, F^d(psi) = c_h^2 B_d);
-// fast magnetosonic speed along D (S3)
+// fast magnetosonic speed along D (S3).  Per state: total pressure pt = p + B^2/2, total energy density
+// E = rho (v^2/2 + e) + B^2/2, B.v and the signal speed; the doubled flux of Eq. 12 is then grouped by
+// state as in the Euler version (A' = v_dr - lambda0, B' = v_dl + lambda0, A = rho_r A', B = rho_l B'):
+//   G_rho = A + B;  G_m,i = A v_ir + B v_il - B_ir B_dr - B_il B_dl (+ pt_l + pt_r for i = d);
+//   G_E = E_r A' + E_l B' + pt_r v_dr + pt_l v_dl - B_dr (B.v)_r - B_dl (B.v)_l;
+//   G_B,i = A' B_ir + B' B_il - B_dr v_ir - B_dl v_il (i != d);  G_B,d = [psi_l + psi_r] - lambda0 (B_dr - B_dl);
+//   G_psi = c_h^2 (B_dl + B_dr) - lambda0 (psi_r - psi_l)
 template <typename T, int D, int NV>
-__device__ __forceinline__ void mhd_state(const T (&W)[NV], const Params<T> &P, T (&U)[NV], T (&F)[NV], T &speed) {
+__device__ __forceinline__ void mhd_scalars(const T (&W)[NV], const Params<T> &P, T &pt, T &E, T &Bv, T &speed) {
   static_assert(NV == 8 || NV == 9, "MHD variable sets");
-  const T rho = W[0], e = W[1], vd = W[2 + D];
-  const T re = rho * e, p = P.gm1 * re, m = rho * vd;
+  const T rho = W[0], e = W[1], vd = W[2 + D], Bd = W[5 + D];
+  const T re = rho * e;
   const T q2 = fma(W[4], W[4], fma(W[3], W[3], W[2] * W[2]));
-  const T Bx = W[5], By = W[6], Bz = W[7], Bd = W[5 + D];
-  const T B2 = fma(Bz, Bz, fma(By, By, Bx * Bx));
-  const T Bv = fma(Bz, W[4], fma(By, W[3], Bx * W[2]));
-  const T hB2 = T(0.5) * B2, pt = p + hB2;
-  const T E = fma(T(0.5) * rho, q2, re) + hB2;
-  U[0] = rho; U[1] = rho * W[2]; U[2] = rho * W[3]; U[3] = rho * W[4]; U[4] = E; U[5] = Bx; U[6] = By; U[7] = Bz;
-  F[0] = m;
-  F[1] = fma(m, W[2], -(Bx * Bd)); F[2] = fma(m, W[3], -(By * Bd)); F[3] = fma(m, W[4], -(Bz * Bd));
-  F[1 + D] += pt;
-  F[4] = fma(E + pt, vd, -(Bd * Bv));
-  F[5] = fma(vd, Bx, -(Bd * W[2])); F[6] = fma(vd, By, -(Bd * W[3])); F[7] = fma(vd, Bz, -(Bd * W[4]));
-  F[5 + D] = T(0);
-  if (NV == 9) {
-    U[8 % NV] = W[8 % NV];
-    F[5 + D] = W[8 % NV];
-    F[8 % NV] = P.ch * P.ch * Bd;
-  }
+  const T B2 = fma(W[7], W[7], fma(W[6], W[6], W[5] * W[5]));
+  Bv = fma(W[7], W[4], fma(W[6], W[3], W[5] * W[2]));
+  const T hB2 = T(0.5) * B2;
+  pt = fma(P.gm1, re, hB2);                                           // Eq. 6 + B^2/2
+  E = fma(T(0.5) * rho, q2, re) + hB2;
   const T ir = frcp(rho);
   const T a2 = P.gg1 * e, s = fma(B2, ir, a2), bd2 = Bd * Bd * ir;
   const T disc = fma(s, s, T(-4) * a2 * bd2);
@@ -186,13 +180,28 @@ __device__ __forceinline__ void mhd_state(const T (&W)[NV], const Params<T> &P, 
 }
 template <typename T, int D, int NV>
 __device__ __forceinline__ void face_flux(const T (&L)[NV], const T (&R)[NV], const Params<T> &P, T (&G)[NV]) {
-  T UL[NV], UR[NV], FL[NV], FR[NV], sl, sr;
-  mhd_state<T, D, NV>(L, P, UL, FL, sl);
-  mhd_state<T, D, NV>(R, P, UR, FR, sr);
+  T ptl, El, Bvl, sl, ptr, Er, Bvr, sr;
+  mhd_scalars<T, D, NV>(L, P, ptl, El, Bvl, sl);
+  mhd_scalars<T, D, NV>(R, P, ptr, Er, Bvr, sr);
   T lam = sl > sr ? sl : sr;
-  if (NV == 9) lam = lam > P.ch ? lam : P.ch;                       // S17
+  if (NV == 9) lam = lam > P.ch ? lam : P.ch;                         // S17
+  const T vdl = L[2 + D], vdr = R[2 + D], Bdl = L[5 + D], Bdr = R[5 + D];
+  const T Ap = vdr - lam, Bp = vdl + lam;
+  const T A = R[0] * Ap, B = L[0] * Bp;
+  G[0] = A + B;
 #pragma unroll
-  for (int v = 0; v < NV; ++v) G[v] = fma(-lam, UR[v] - UL[v], FL[v] + FR[v]);
+  for (int t = 0; t < 3; ++t) {
+    T x = fma(-L[5 + t], Bdl, B * L[2 + t]);
+    if (t == D) x += ptl + ptr;
+    G[1 + t] = fma(A, R[2 + t], fma(-R[5 + t], Bdr, x));
+    G[5 + t] = t == D ? -(lam * (Bdr - Bdl))
+                      : fma(Ap, R[5 + t], fma(Bp, L[5 + t], fma(-Bdr, R[2 + t], -(Bdl * L[2 + t]))));
+  }
+  G[4] = fma(Er, Ap, fma(El, Bp, fma(ptr, vdr, fma(ptl, vdl, fma(-Bdr, Bvr, -(Bdl * Bvl))))));
+  if (NV == 9) {
+    G[5 + D] += L[8 % NV] + R[8 % NV];
+    G[8 % NV] = fma(P.ch * P.ch, Bdl + Bdr, -(lam * (R[8 % NV] - L[8 % NV])));
+  }
 }
 
 // fp32: the same value from the 3-input min/max of sm_100 (FMNMX3): with x = 2 theta dm, y = 2 theta dp,
