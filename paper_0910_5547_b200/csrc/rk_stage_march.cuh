@@ -260,6 +260,9 @@ template <typename T> struct Cfg;
 template <> struct Cfg<double> { static constexpr int PW = 21, PQ = 17, PY = 16, NSLOT = AMR_NSLOT64; };
 template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18, NSLOT = AMR_NSLOT32; };
 
+#ifndef AMR_BASE_TMA
+#define AMR_BASE_TMA 1      // combination stage: U_base planes come through their own TMA ring (no global loads in the warps)
+#endif
 // LITE: register-light layout for two CTAs per SM (rk_stage_lite.cuh): 3-slot ring, the flux
 // arrays alias the q+ arrays (slot s is read as q+ by its only reader before that same thread
 // overwrites it with the flux), plus per-thread slots for the z-marching state.
@@ -273,7 +276,13 @@ template <typename T, int NV, bool LITE = false> struct Smem {
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
                        O_FX = LITE ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
                        O_FY = LITE ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV,
-                       O_QPZ = O_ACC + (LITE ? NV * ACV : 0), O_END = O_QPZ + (LITE ? NV * ACV : 0);
+                       O_QPZ = O_ACC + (LITE ? NV * ACV : 0);
+  // fp64: ring of U_base planes for the combination stage (128-byte aligned TMA destination); fp32 keeps
+  // plain loads, the extra 20 kB would cost its third CTA per SM
+  static constexpr int O_BRAW = ((O_QPZ + (LITE ? NV * ACV : 0) + 31) / 32) * 32;
+  static constexpr bool BTMA = !LITE && AMR_BASE_TMA && sizeof(T) == 8 &&
+                               size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, MHD does not)
+  static constexpr int O_END = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
   static constexpr size_t BYTES = BAR_OFF + NSLOT * 8 + 128;   // + slack to align the ring to 128 B
 };
@@ -295,7 +304,7 @@ template <typename T, int NV, int D, typename S = Smem<T, NV>>
 __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int lane, const Params<T> &P, T th2,
                                           T *__restrict__ bflux, int pl, int &hits, bool producer,
                                           const CUtensorMap *tmap, unsigned long long *bars, int q_mid, int q_lo,
-                                          int q_hi, int kz_lo, int kz_hi) {
+                                          int q_hi, int kz_lo, int kz_hi, int q_base = -1) {
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
   constexpr int gst = D == 0 ? 1 : PX, rst = D == 0 ? 1 : PW;
@@ -336,8 +345,11 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
     const int slot = pk % S::NSLOT;
     const int q = pk < NG ? q_lo : (pk >= NG + NI ? q_hi : q_mid);
     const int k = pk < NG ? pk + kz_lo : (pk >= NG + NI ? pk + kz_hi : pk);
-    mbar_expect_tx(&bars[slot], unsigned(S::RAWP * sizeof(T)));
+    // U_base of cell pk-2 rides on the same barrier: it is needed when plane pk has been converted (Eq. 8)
+    const bool wb = q_base >= 0 && pk >= NG + 2;
+    mbar_expect_tx(&bars[slot], unsigned(S::RAWP * sizeof(T)) * (wb ? 2u : 1u));
     tma_load_4d(sm + S::O_RAW + slot * S::RAWP, tmap, 0, NG, k, q, &bars[slot]);
+    if (wb) tma_load_4d(sm + S::O_BRAW + slot * S::RAWP, tmap, 0, NG, pk - 2, q_base, &bars[slot]);
   };
   if (producer) {
 #pragma unroll
@@ -470,7 +482,9 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
       T ub[NV];
       if (BASE && c > NG) {
 #pragma unroll
-        for (int v = 0; v < NV; ++v) ub[v] = base[size_t(v) * VS + (c - 1) * PLANE];
+        for (int v = 0; v < NV; ++v)
+          ub[v] = S::BTMA ? raw[S::O_BRAW - S::O_RAW + ((c + 1) % S::NSLOT) * RAWP + v * (NI * NI)]   // arrived with plane c+1
+                               : base[size_t(v) * VS + (c - 1) * PLANE];
       }
       // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
       T Gz[NV];
@@ -587,7 +601,8 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     const int q_mid = (qbase + p) * NV, q_lo = (qbase + (nzl >= 0 ? nzl : p)) * NV, q_hi = (qbase + (nzh >= 0 ? nzh : p)) * NV;
     const int kz_lo = nzl >= 0 ? NI : 0, kz_hi = nzh >= 0 ? -NI : 0;
     if (warp == 8)
-      mk::halo_warp<T, NV, 0>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
+      mk::halo_warp<T, NV, 0>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi,
+                              (BASE && S::BTMA) ? (sbase * pool.max_patches + p) * NV : -1);
     else
       mk::halo_warp<T, NV, 1>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
   }
