@@ -109,3 +109,27 @@ def test_sedov_amr_fp32_and_direct_halos(gpu, dtype, halo):
     G, O = g.download(0).astype(np.float64), o.download(0)
     assert np.isfinite(G).all()
     assert norm_err(G, O, vector=(dtype == "f32")).max() <= (1e-12 if dtype == "f64" else 1e-5)
+
+
+@pytest.mark.parametrize("dtype,nv", [("f64", 5), ("f32", 5), ("f64", 8), ("f64", 9)])
+def test_whole_path_is_bitwise_reproducible(gpu, dtype, nv):
+    """Race detector of last resort (compute-sanitizer is closed on this pool): the same inputs through the
+    whole path three times, on a grid of several waves of CTAs and on an AMR hierarchy, give the same bits."""
+    cases = [(wl.uniform_hierarchy(4, periodic=True), dict(halo=1)), (wl.ball_hierarchy(2, 4, bc=(1,) * 6), dict(halo=1)),
+             (wl.ball_hierarchy(2, 3, bc=(1,) * 6), dict(halo=0))]
+    for h, kw in cases:
+        U = rand_state(h, nv, 17)
+        if nv == 9:
+            U = np.concatenate([U, 0.05 * np.random.default_rng(18).standard_normal(U[:, :1].shape)], axis=1)
+        outs = []
+        for rep in range(3):
+            g = gpu.AmrHydro(h, 1.4, nv, dtype=dtype, **kw)
+            g.upload(0, U)
+            if h["nlevels"] > 1:
+                for lev in range(h["nlevels"] - 1, 0, -1):
+                    g.restrict(lev)
+            for _ in range(3):
+                g.advance(0.3)
+            outs.append(g.download(0))
+            assert np.isfinite(outs[-1]).all()
+        assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
