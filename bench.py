@@ -348,7 +348,8 @@ def run_ours(args):
             "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_per_step,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
             "data": "synthetic",
-            "config": {"workload": w["name"], "patches": npatch, "cells": npatch * 4096, "nvars": nv,
+            "config": {"workload": w["name"] if not args.size or args.size == w["size"] else
+                       w["name"] + " (REDUCED to %d cells per side by --size)" % args.size, "patches": npatch, "cells": npatch * 4096, "nvars": nv,
                        "cfl": cfl, "halo": "direct sibling reads" if args.halo else "materialised ghosts",
                        "l2_policy": "working set (%.1f GB per slot) far exceeds the 126 MB L2" % (npatch * nv * 4096 * esz / 1e9)
                        if npatch * nv * 4096 * esz > 4 * 126e6 else "working set fits L2 (small config)",
