@@ -266,7 +266,7 @@ template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18, 
 // LITE: register-light layout for two CTAs per SM (rk_stage_lite.cuh): 3-slot ring, the flux
 // arrays alias the q+ arrays (slot s is read as q+ by its only reader before that same thread
 // overwrites it with the flux), plus per-thread slots for the z-marching state.
-template <typename T, int NV, bool LITE = false> struct Smem {
+template <typename T, int NV, bool LITE = false, bool WB = true> struct Smem {   // WB: the kernel reads U_base (combination stage)
   static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY, NSLOT = LITE ? 3 : Cfg<T>::NSLOT;
   static constexpr int RAWP = NV * NI * NI;        // one raw plane: [NV][16][16], dense TMA box
   static constexpr int WV = NP * PW;               // one variable of one primitive plane [20][PW]
@@ -277,11 +277,11 @@ template <typename T, int NV, bool LITE = false> struct Smem {
                        O_FX = LITE ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
                        O_FY = LITE ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV,
                        O_QPZ = O_ACC + (LITE ? NV * ACV : 0);
-  // fp64: ring of U_base planes for the combination stage (128-byte aligned TMA destination); fp32 keeps
-  // plain loads, the extra 20 kB would cost its third CTA per SM
+  // ring of U_base planes for the combination stage (128-byte aligned TMA destination).  fp32 Euler: the extra
+  // 20 kB cost the third CTA per SM, so that instantiation also takes 96 registers instead of 64 (launch bounds)
   static constexpr int O_BRAW = ((O_QPZ + (LITE ? NV * ACV : 0) + 31) / 32) * 32;
-  static constexpr bool BTMA = !LITE && AMR_BASE_TMA && sizeof(T) == 8 &&
-                               size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, MHD does not)
+  static constexpr bool BTMA = !LITE && WB && AMR_BASE_TMA && (sizeof(T) == 8 || NV == 5) &&
+                               size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, fp64 MHD does not)
   static constexpr int O_END = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
   static constexpr size_t BYTES = BAR_OFF + NSLOT * 8 + 128;   // + slack to align the ring to 128 B
@@ -398,11 +398,11 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
 }  // namespace mk
 
 template <typename T, int NV, bool BASE>
-__global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? AMR_MINB32 : 2)))
+__global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? (BASE && AMR_BASE_TMA ? 2 : AMR_MINB32) : 2)))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
                  const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out) {
-  using S = mk::Smem<T, NV>;
+  using S = mk::Smem<T, NV, false, BASE>;
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
   extern __shared__ unsigned char smem_raw[];
@@ -601,10 +601,10 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     const int q_mid = (qbase + p) * NV, q_lo = (qbase + (nzl >= 0 ? nzl : p)) * NV, q_hi = (qbase + (nzh >= 0 ? nzh : p)) * NV;
     const int kz_lo = nzl >= 0 ? NI : 0, kz_hi = nzh >= 0 ? -NI : 0;
     if (warp == 8)
-      mk::halo_warp<T, NV, 0>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi,
+      mk::halo_warp<T, NV, 0, S>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi,
                               (BASE && S::BTMA) ? (sbase * pool.max_patches + p) * NV : -1);
     else
-      mk::halo_warp<T, NV, 1>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
+      mk::halo_warp<T, NV, 1, S>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
   }
   if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
 }
@@ -642,19 +642,19 @@ int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sb
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
                           cudaStream_t stream, unsigned long long *smax_out = nullptr) {
   static bool configured = false;
-  constexpr size_t bytes = mk::Smem<T, NV>::BYTES;
+  constexpr size_t bytes0 = mk::Smem<T, NV, false, false>::BYTES, bytes1 = mk::Smem<T, NV, false, true>::BYTES;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+    cudaError_t e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+      e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes1));
     if (e != cudaSuccess) return int(e);
     configured = true;
   }
   if (a != T(0))
-    k_rk_stage_march<T, NV, true><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
+    k_rk_stage_march<T, NV, true><<<n, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
                                                                      floor_hits, desc, direct_halo, smax_out);
   else
-    k_rk_stage_march<T, NV, false><<<n, mk::THREADS, bytes, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
+    k_rk_stage_march<T, NV, false><<<n, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
                                                                       floor_hits, desc, direct_halo, nullptr);
   return 0;
 }
