@@ -273,9 +273,11 @@ template <typename T, int NV, bool LITE = false, bool WB = true> struct Smem {  
   static constexpr int QXV = NI * PQ;              // [16][PQ]: slot s = q+ of cell s-1 / flux at face s
   static constexpr int QYV = (NI + 1) * PY;        // [17][PY]
   static constexpr int ACV = NI * NI;              // per-thread slots, indexed by (warp, lane)
+  // the flux arrays alias the q+ arrays in LITE, and in the fp64 MHD combination stage so that its U_base ring fits
+  static constexpr bool ALIAS = LITE || (WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 8);
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
-                       O_FX = LITE ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
-                       O_FY = LITE ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV,
+                       O_FX = ALIAS ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
+                       O_FY = ALIAS ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV,
                        O_QPZ = O_ACC + (LITE ? NV * ACV : 0);
   // ring of U_base planes for the combination stage (128-byte aligned TMA destination).  fp32 Euler: the extra
   // 20 kB cost the third CTA per SM, so that instantiation also takes 96 registers instead of 64 (launch bounds)
