@@ -69,6 +69,10 @@ extern "C" {
 #define AMRHYDRO_OPT_GLM_CR 9     /* nvars = 9: c_r = c_p^2/c_h of the psi damping applied by amrhydro_advance
                                      (S18), default 0.18, 0 = none; any time                               */
 
+#define AMRHYDRO_OPT_ZSPLIT 10     /* default rk_stage kernel: two CTAs per patch, each marching over half of the column
+                                     (3 warm-up planes more per CTA, about half the latency of a launch):
+                                     0 = never, 1 = always, 2 (default) = on levels of at most SMs/2 patches; any time */
+
 /* counters (amrhydro_get_counter) */
 #define AMRHYDRO_CNT_LAUNCHES 1   /* kernels launched by this handle since create / last reset */
 #define AMRHYDRO_CNT_FLOOR_HITS 2 /* cells/states where a floor of S11 was applied (rk_stage, cfl) */

@@ -49,6 +49,8 @@ struct amrhydro {
   unsigned long long *d_scalars = nullptr;  // [0] scratch, [1] floor hits
   unsigned long long *d_smax = nullptr;     // per level: bits of the max signal speed of (level, smax_slot[level])
   std::vector<int> smax_slot;               // slot the cached value belongs to, -1 = stale
+  int zsplit = 2;                           // rk_stage_march: 0 never, 1 always, 2 = levels of at most num_sms/2 patches
+  int num_sms = 148;
   int fuse_cfl = 2;                         // 0 never, 1 always, 2 = where it is free (fp32)
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
@@ -157,6 +159,11 @@ amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) 
   amrhydro *h = new amrhydro;
   h->gamma = gamma;
   h->nv = nvars;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      h->num_sms = sms;
+  }
   if (cudaMalloc(&h->d_scalars, 2 * sizeof(unsigned long long)) != cudaSuccess) { delete h; return nullptr; }
   cudaMemset(h->d_scalars, 0, 2 * sizeof(unsigned long long));
   return h;
@@ -206,6 +213,10 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
     case AMRHYDRO_OPT_GLM_CR:
       if (!(value >= 0.0) || !std::isfinite(value)) return fail(h, AMRHYDRO_EINVAL, "c_r must be >= 0 and finite");
       h->glm_cr = value;
+      return 0;
+    case AMRHYDRO_OPT_ZSPLIT:
+      if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "zsplit must be 0, 1 or 2");
+      h->zsplit = int(value);
       return 0;
     case AMRHYDRO_OPT_FUSE_CFL:
       if (value != 0 && value != 1 && value != 2) return fail(h, AMRHYDRO_EINVAL, "fuse_cfl must be 0, 1 or 2");
@@ -538,7 +549,8 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                           fuse ? h->d_smax + level : nullptr);
+                                           fuse ? h->d_smax + level : nullptr,
+                                           (h->zsplit == 1 || (h->zsplit == 2 && 2 * n <= h->num_sms)) ? 1 : 0);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
       if (fuse) h->smax_slot[level] = sout;

@@ -306,7 +306,9 @@ template <typename T, int NV, int D, typename S = Smem<T, NV>>
 __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int lane, const Params<T> &P, T th2,
                                           T *__restrict__ bflux, int pl, int &hits, bool producer,
                                           const CUtensorMap *tmap, unsigned long long *bars, int q_mid, int q_lo,
-                                          int q_hi, int kz_lo, int kz_hi, int q_base = -1) {
+                                          int q_hi, int kz_lo, int kz_hi, int q_base = -1, int zlo = 0, int nz = NI) {
+  // zlo, nz: the CTA marches over the nz cells starting at cell zlo of the column (z-split of small levels); plane
+  // indices below are relative to that start, zlo converts them to planes of the patch
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
   constexpr int gst = D == 0 ? 1 : PX, rst = D == 0 ? 1 : PW;
@@ -326,7 +328,7 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
   auto load = [&](int pk) {
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      const T *s = g + size_t(v) * VS + pk * PLANE;
+      const T *s = g + size_t(v) * VS + (pk + zlo) * PLANE;
       if (D == 0) {
         if (sizeof(T) == 8) { const double2 x = *reinterpret_cast<const double2 *>(s); Ua[v] = T(x.x); Ub[v] = T(x.y); }
         else                { const float2 x = *reinterpret_cast<const float2 *>(s);   Ua[v] = T(x.x); Ub[v] = T(x.y); }
@@ -345,13 +347,14 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
   };
   auto issue = [&](int pk) {                                  // TMA: interior box of padded plane pk
     const int slot = pk % S::NSLOT;
-    const int q = pk < NG ? q_lo : (pk >= NG + NI ? q_hi : q_mid);
-    const int k = pk < NG ? pk + kz_lo : (pk >= NG + NI ? pk + kz_hi : pk);
+    const int ap = pk + zlo;
+    const int q = ap < NG ? q_lo : (ap >= NG + NI ? q_hi : q_mid);
+    const int k = ap < NG ? ap + kz_lo : (ap >= NG + NI ? ap + kz_hi : ap);
     // U_base of cell pk-2 rides on the same barrier: it is needed when plane pk has been converted (Eq. 8)
     const bool wb = q_base >= 0 && pk >= NG + 2;
     mbar_expect_tx(&bars[slot], unsigned(S::RAWP * sizeof(T)) * (wb ? 2u : 1u));
     tma_load_4d(sm + S::O_RAW + slot * S::RAWP, tmap, 0, NG, k, q, &bars[slot]);
-    if (wb) tma_load_4d(sm + S::O_BRAW + slot * S::RAWP, tmap, 0, NG, pk - 2, q_base, &bars[slot]);
+    if (wb) tma_load_4d(sm + S::O_BRAW + slot * S::RAWP, tmap, 0, NG, ap - 2, q_base, &bars[slot]);
   };
   if (producer) {
 #pragma unroll
@@ -363,10 +366,10 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
   __syncthreads();                                            // planes 0-2 converted by the interior warps
   if (producer) issue(S::NSLOT);                              // slot of plane 0: converted, never needed again
 #pragma unroll 1
-  for (int c = NG; c < NG + NI; ++c) {
-    if (c + 1 < NG + NI) {
+  for (int c = NG; c < NG + nz; ++c) {
+    if (c + 1 < NG + nz) {
       publish(c + 1);
-      if (c + 2 < NG + NI) load(c + 2);
+      if (c + 2 < NG + nz) load(c + 2);
     }
     const T *s3 = st3 + (c & 1) * (NV * WV);
     T qm[NV];
@@ -378,7 +381,7 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
       if (!hi) qlo[v * qv] = fma(q4, s, w1);                  // q+ of cell -1 (low side)
     }
     __syncthreads();
-    if (producer && c + S::NSLOT - 1 < NP) issue(c + S::NSLOT - 1);   // slot of plane c-1 is free: cell c-1 is finished
+    if (producer && c + S::NSLOT - 1 < nz + 2 * NG) issue(c + S::NSLOT - 1);   // slot of plane c-1 is free: cell c-1 is finished
     if (hi) {
       T WL[NV], G[NV];
 #pragma unroll
@@ -388,7 +391,7 @@ __device__ __forceinline__ void halo_warp(T *sm, const T *glo, const T *ghi, int
 #pragma unroll
       for (int v = 0; v < NV; ++v) fhi[v * qv] = G[v];
       if (bflux) {
-        T *B = bflux + ((size_t(pl) * 9 + 3 * D + 2) * NV) * 256 + (c - NG) * 16 + t;
+        T *B = bflux + ((size_t(pl) * 9 + 3 * D + 2) * NV) * 256 + (c - NG + zlo) * 16 + t;
 #pragma unroll
         for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
       }
@@ -403,7 +406,7 @@ template <typename T, int NV, bool BASE>
 __global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? (BASE && AMR_BASE_TMA ? 2 : AMR_MINB32) : 2)))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out) {
+                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit) {
   using S = mk::Smem<T, NV, false, BASE>;
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
@@ -412,7 +415,9 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
   T *sm = reinterpret_cast<T *>(smem_raw + ((128u - (mk::smem_u32(smem_raw) & 127u)) & 127u));
   unsigned long long *bars = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(sm) + S::BAR_OFF);
 
-  const int pl = blockIdx.x, p = first + pl;
+  // zsplit = 1 (levels too small to fill the machine): two CTAs per patch, each marching over 8 of the 16 cells in z
+  const int pl = blockIdx.x >> zsplit, p = first + pl;
+  const int zlo = int(blockIdx.x & zsplit) * (NI / 2), nz = zsplit ? NI / 2 : NI;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
   const T th2 = T(2) * P.theta, q4 = T(0.25);
@@ -457,7 +462,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         wme[v * WV] = Wc[v];                                        // plane 2 -> primitive buffer 0
         const T dm = W1[v] - W0[v];
         dzm[v] = Wc[v] - W1[v];
-        const T s = mk::slope4(dm, dzm[v], Wc[v] - W0[v], th2);
+        const T s = mk::slope4(dm, dzm[v], dm + dzm[v], th2);            // (the sum, as in the loop: a z-split march must give the same bits)
         qpz[v] = fma(q4, s, W1[v]);                                 // q+ of the ghost cell below plane 2
         acc[v] = T(0);
       }
@@ -465,7 +470,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     __syncthreads();
 
 #pragma unroll 1
-    for (int c = NG; c <= NG + NI; ++c) {            // current cell = padded plane c (2..17); c = 18: last z face only
+    for (int c = NG; c <= NG + nz; ++c) {            // current cell = plane c of this march (2..nz+1); c = nz+2: last z face only
       // 1. plane c+1: raw -> primitives, publish for the x/y neighbours
       T Wn[NV];
       {
@@ -476,7 +481,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         for (int v = 0; v < NV; ++v) Un[v] = raw[slot * RAWP + v * (NI * NI)];
         mk::prim<T, NV>(Un, Wn, P, hits);
       }
-      if (c + 1 < NG + NI) {
+      if (c + 1 < NG + nz) {
         T *w = wme + ((c + 1) & 1) * (NV * WV);
 #pragma unroll
         for (int v = 0; v < NV; ++v) w[v * WV] = Wn[v];
@@ -486,7 +491,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
 #pragma unroll
         for (int v = 0; v < NV; ++v)
           ub[v] = S::BTMA ? raw[S::O_BRAW - S::O_RAW + ((c + 1) % S::NSLOT) * RAWP + v * (NI * NI)]   // arrived with plane c+1
-                               : base[size_t(v) * VS + (c - 1) * PLANE];
+                               : base[size_t(v) * VS + (c - 1 + zlo) * PLANE];
       }
       // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
       T Gz[NV];
@@ -505,14 +510,14 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
 #pragma unroll
         for (int v = 0; v < NV; ++v) qpz[v] = qp[v];
       }
-      if (bflux && ((c - NG) & 7) == 0) {
-        T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG) >> 3)) * NV) * 256 + j * 16 + i;
+      if (bflux && ((c - NG + zlo) & 7) == 0) {
+        T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG + zlo) >> 3)) * NV) * 256 + j * 16 + i;
 #pragma unroll
         for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gz[v];
       }
       if (c > NG) {
         const T *ui = raw + ((c - 1) % S::NSLOT) * RAWP;     // raw U of cell c-1 is still in the ring
-        T *o = out + (c - 1) * PLANE;
+        T *o = out + (c - 1 + zlo) * PLANE;
         T un[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
@@ -531,7 +536,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
           best = tmax(best, sp);
         }
       }
-      if (c < NG + NI) {
+      if (c < NG + nz) {
         // 3. x/y phase 1: slopes of this cell along x and y, publish q+
         const T *w = wme + (c & 1) * (NV * WV);
         T qmx[NV], qmy[NV];
@@ -560,12 +565,12 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         }
         if (bflux) {
           if ((i & 7) == 0) {
-            T *B = bflux + ((size_t(pl) * 9 + 0 + (i >> 3)) * NV) * 256 + (c - NG) * 16 + j;
+            T *B = bflux + ((size_t(pl) * 9 + 0 + (i >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + j;
 #pragma unroll
             for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx[v];
           }
           if ((j & 7) == 0) {
-            T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG) * 16 + i;
+            T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + i;
 #pragma unroll
             for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gy[v];
           }
@@ -604,9 +609,10 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     const int kz_lo = nzl >= 0 ? NI : 0, kz_hi = nzh >= 0 ? -NI : 0;
     if (warp == 8)
       mk::halo_warp<T, NV, 0, S>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, lane == 0, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi,
-                              (BASE && S::BTMA) ? (sbase * pool.max_patches + p) * NV : -1);
+                              (BASE && S::BTMA) ? (sbase * pool.max_patches + p) * NV : -1, zlo, nz);
     else
-      mk::halo_warp<T, NV, 1, S>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi);
+      mk::halo_warp<T, NV, 1, S>(sm, g[0], g[1], lane, P, th2, bflux, pl, hits, false, &tmap, bars, q_mid, q_lo, q_hi, kz_lo, kz_hi,
+                                 -1, zlo, nz);
   }
   if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
 }
@@ -642,7 +648,7 @@ int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int ns
 template <typename T, int NV>
 int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                          cudaStream_t stream, unsigned long long *smax_out = nullptr) {
+                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0) {
   static bool configured = false;
   constexpr size_t bytes0 = mk::Smem<T, NV, false, false>::BYTES, bytes1 = mk::Smem<T, NV, false, true>::BYTES;
   if (!configured) {
@@ -653,11 +659,11 @@ int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sb
     configured = true;
   }
   if (a != T(0))
-    k_rk_stage_march<T, NV, true><<<n, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
-                                                                     floor_hits, desc, direct_halo, smax_out);
+    k_rk_stage_march<T, NV, true><<<n << zsplit, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                                bflux, floor_hits, desc, direct_halo, smax_out, zsplit);
   else
-    k_rk_stage_march<T, NV, false><<<n, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P, bflux,
-                                                                      floor_hits, desc, direct_halo, nullptr);
+    k_rk_stage_march<T, NV, false><<<n << zsplit, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                                 bflux, floor_hits, desc, direct_halo, nullptr, zsplit);
   return 0;
 }
 

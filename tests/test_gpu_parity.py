@@ -205,6 +205,27 @@ def test_rk_stage_with_active_floors(gpu, kernel, halo):
     assert norm_err(g.download(0), o.download(0)).max() <= 1e-12
 
 
+@pytest.mark.parametrize("nv,dtype", [(5, "f64"), (5, "f32"), (8, "f64"), (9, "f64")])
+@pytest.mark.parametrize("halo", [0, 1])
+def test_rk_stage_zsplit_bitwise_equal(gpu, nv, dtype, halo):
+    """AMRHYDRO_OPT_ZSPLIT: two CTAs per patch march over half a column each; same arithmetic per cell, so the
+    results (and the flux registers of an AMR level) are bitwise those of the one-CTA march."""
+    h = amr_hier("slab")
+    U = rand_state(h, nv, 51, 5.0 / 3.0)
+    out = []
+    for zs in (0, 1):
+        g = gpu.AmrHydro(h, 5.0 / 3.0, nv, dtype=dtype, halo=halo, zsplit=zs)
+        g.upload(0, U)
+        g.restrict(1)
+        for _ in range(2):
+            g.advance(0.3)
+        regs = [g.download_registers(int(p)) for p in wl.level_patches(h, 1)[:4]]
+        out.append((g.download(0), regs))
+    assert np.array_equal(out[0][0], out[1][0]) and np.isfinite(out[0][0]).all()
+    for (a, b), (c, d) in zip(out[0][1], out[1][1]):
+        assert np.array_equal(a, c) and np.array_equal(b, d)
+
+
 def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
     h = wl.uniform_hierarchy(2, periodic=False)
     U = rand_state(h, 5, 8)
