@@ -10,11 +10,18 @@
 //    over the 20 padded planes; warp 8 owns the x-halo columns, warp 9 the y-halo rows.
 //    Fluxes, L(U) and primitives never touch HBM.
 //  * the 16x16xNV interior box of every plane is brought in by TMA (cp.async.bulk.tensor, one
-//    request per plane, 3-slot ring, mbarrier completion), issued two planes ahead by one
+//    request per plane, 4-slot ring, mbarrier completion), issued three planes ahead by one
 //    elected thread: no load instructions, address arithmetic or prefetch registers in the
 //    interior warps, and the raw U of the cell being finished is still in the ring for the
 //    Runge-Kutta combination.  z-ghost planes come through the same ring (from this patch's ghost
-//    zones, or with AMRHYDRO_OPT_HALO=1 from the z-neighbour's interior).
+//    zones, or with AMRHYDRO_OPT_HALO=1 from the z-neighbour's interior).  In the combination
+//    stage (a != 0) the planes of U_base ride on the same mbarriers into a second ring (fp64 and
+//    fp32 Euler, fp64 8-variable MHD with the flux arrays aliased onto the q+ arrays): measured
+//    -14 % on that stage against 5 global loads per cell in the warps.  Shared-memory layout and
+//    launch bounds are per stage (fp32: 3 CTAs/SM at 64 registers without the ring, 2 at 96 with it).
+//  * optional extras, all bitwise-neutral for the state: the CFL reduction of the next step fused
+//    into the combination stage (smax_out); a z-split for levels too small to fill the machine
+//    (two CTAs per patch, half a column each, about half the latency of a launch).
 //  * each cell is converted to primitives once (one MUFU reciprocal + a third-order correction)
 //    and published in a double-buffered shared-memory plane for the x/y neighbours; the z stencil
 //    lives in registers; x/y exchange the cell-edge state q+ and the face fluxes through shared
