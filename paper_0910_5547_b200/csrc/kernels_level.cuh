@@ -114,6 +114,9 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   T *U = pool.patch(slot, p);
   __shared__ int s_nbr[27];
   __shared__ int s_org[3], s_porg[3];
+  // the parent cells this plane prolongates from, time-interpolated once (S7): 3 coarse planes x 12 x 12 per variable
+  constexpr int CT = 12, CTV = 3 * CT * CT;
+  __shared__ T s_par[NV * CTV];
   if (threadIdx.x < 27) s_nbr[threadIdx.x] = D.nbr[threadIdx.x];
   if (threadIdx.x < 3) {
     s_org[threadIdx.x] = D.origin[threadIdx.x];
@@ -121,10 +124,30 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   }
   __syncthreads();
   const int Q = D.parent;
-  const T *Co = Q >= 0 ? pool.patch(pold, Q) : nullptr;
-  const T *Cn = Q >= 0 ? pool.patch(pnew, Q) : nullptr;
-  const bool only_old = alpha == T(0), only_new = alpha == T(1);
   const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
+  bool cf = false;                                   // block-uniform: does this plane touch a coarse-fine region?
+  if (Q >= 0) {
+#pragma unroll
+    for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && s_nbr[(oz + 1) * 9 + r] == -1;
+  }
+  int pc0[3] = {0, 0, 0};                            // parent padded index of the tile's first cell
+  if (cf) {
+    const T *Co = pool.patch(pold, Q), *Cn = pool.patch(pnew, Q);
+    const bool only_old = alpha == T(0), only_new = alpha == T(1);
+#pragma unroll
+    for (int d = 0; d < 2; ++d) pc0[d] = s_org[d] / 2 - s_porg[d] + NG - 2;          // covers fine ghosts and the slope stencil
+    {
+      const int g = s_org[2] + k - NG;
+      pc0[2] = ((g + 64) / 2 - 32) - s_porg[2] + NG - 1;
+    }
+    for (int t = threadIdx.x; t < NV * CTV; t += 256) {
+      const int v = t / CTV, r = t % CTV;
+      const int c = cell<T>(pc0[2] + r / (CT * CT), pc0[1] + (r / CT) % CT, pc0[0] + r % CT);
+      const T *o = Co + size_t(v) * Layout<T>::VS, *n = Cn + size_t(v) * Layout<T>::VS;
+      s_par[t] = only_old ? o[c] : (only_new ? n[c] : (T(1) - alpha) * o[c] + alpha * n[c]);
+    }
+    __syncthreads();
+  }
   // ghost cells of this plane: all 400 on a z-ghost plane, else the 144 of the frame
   const int ncell = oz != 0 ? NP * NP : NP * NP - NI * NI;
   for (int t = threadIdx.x; t < ncell; t += 256) {
@@ -145,33 +168,24 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
       for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + me] = S[size_t(v) * Layout<T>::VS + sc];
     } else if (nb == -1 && Q >= 0) {
       const int pad[3] = {i, j, k};
-      int pc[3];
+      int lc[3];
       T s[3];
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         const int g = s_org[d] + pad[d] - NG;        // fine global index (>= -2)
         const int gc = (g + 64) / 2 - 32;            // floor(g/2) for g >= -64
         s[d] = (g - 2 * gc == 0) ? T(-0.25) : T(0.25);
-        pc[d] = gc - s_porg[d] + NG;
+        lc[d] = gc - s_porg[d] + NG - pc0[d];        // index in the staged tile
       }
-      const int c0 = cell<T>(pc[2], pc[1], pc[0]);
-      const int st[3] = {1, Layout<T>::PX, Layout<T>::PLANE};
+      const int c0 = (lc[2] * CT + lc[1]) * CT + lc[0];
+      const int st[3] = {1, CT, CT * CT};
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
-        const T *o = Co + size_t(v) * Layout<T>::VS, *n = Cn + size_t(v) * Layout<T>::VS;
-        auto at = [&](int c) {
-          if (only_old) return o[c];
-          if (only_new) return n[c];
-          return (T(1) - alpha) * o[c] + alpha * n[c];
-        };
-        const T uc = at(c0);
+        const T *c = s_par + v * CTV;
+        const T uc = c[c0];
         T val = uc;
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-          const T up = at(c0 + st[d]);
-          const T um = at(c0 - st[d]);
-          val = val + s[d] * minmod2(up - uc, uc - um);
-        }
+        for (int d = 0; d < 3; ++d) val = val + s[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
         U[size_t(v) * Layout<T>::VS + me] = val;
       }
     }
