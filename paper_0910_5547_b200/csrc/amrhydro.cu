@@ -499,7 +499,7 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
     constexpr int NV = decltype(nv)::value;
     if (phase1) {
       k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
-          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, skip);
+          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, skip);
       LAUNCH_CHECK(h);
     }
     if (phase2) {

@@ -108,86 +108,95 @@ template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
 // outflow, x then y then z over the full padded extent, one block per patch.
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
-                                                     int first, const Desc *__restrict__ desc, int skip_siblings) {
+                                                     int first, const Desc *__restrict__ desc,
+                                                     const int *__restrict__ octant, int skip_siblings) {
+  // Latency is what this kernel costs on small AMR levels, so it is written as two dependent round trips to
+  // memory: (1) the patch's descriptor row and octant (every thread reads what it needs, broadcast through
+  // L1: no staging, no barrier), (2) all parent cells this plane prolongates from -- 3 coarse planes x 12 x 12
+  // per variable, time-interpolated once (S7) into shared memory -- together with the sibling cells to copy.
+  // A fine patch is an octant of its parent and origins are multiples of 16, so parent indices follow from
+  // the octant bits alone: coarse index of padded fine index t along d = 8 oc_d + floor((t - 2) / 2) + 2.
   const int p = first + blockIdx.x, k = blockIdx.y;
   const Desc &D = desc[p];
   T *U = pool.patch(slot, p);
-  __shared__ int s_nbr[27];
-  __shared__ int s_org[3], s_porg[3];
-  // the parent cells this plane prolongates from, time-interpolated once (S7): 3 coarse planes x 12 x 12 per variable
   constexpr int CT = 12, CTV = 3 * CT * CT;
   __shared__ T s_par[NV * CTV];
-  if (threadIdx.x < 27) s_nbr[threadIdx.x] = D.nbr[threadIdx.x];
-  if (threadIdx.x < 3) {
-    s_org[threadIdx.x] = D.origin[threadIdx.x];
-    s_porg[threadIdx.x] = D.parent >= 0 ? desc[D.parent].origin[threadIdx.x] : 0;
-  }
-  __syncthreads();
   const int Q = D.parent;
   const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
+  const int *nbr = D.nbr + (oz + 1) * 9;             // the nine regions of this plane
   bool cf = false;                                   // block-uniform: does this plane touch a coarse-fine region?
   if (Q >= 0) {
 #pragma unroll
-    for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && s_nbr[(oz + 1) * 9 + r] == -1;
+    for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
   }
   int pc0[3] = {0, 0, 0};                            // parent padded index of the tile's first cell
   if (cf) {
+    const int o = octant[p];
+    pc0[0] = 8 * (o & 1) + NG - 2;                   // covers the fine ghosts and the slope stencil
+    pc0[1] = 8 * ((o >> 1) & 1) + NG - 2;
+    pc0[2] = 8 * ((o >> 2) & 1) + ((k - NG + 64) / 2 - 32) + NG - 1;
     const T *Co = pool.patch(pold, Q), *Cn = pool.patch(pnew, Q);
     const bool only_old = alpha == T(0), only_new = alpha == T(1);
+    // 432 tile cells per variable over 256 threads: two cells per thread, their parent offsets computed once
+    const int r0 = threadIdx.x, r1 = threadIdx.x + 256;
+    const int c0 = cell<T>(pc0[2] + r0 / (CT * CT), pc0[1] + (r0 / CT) % CT, pc0[0] + r0 % CT);
+    const int c1 = r1 < CTV ? cell<T>(pc0[2] + r1 / (CT * CT), pc0[1] + (r1 / CT) % CT, pc0[0] + r1 % CT) : -1;
 #pragma unroll
-    for (int d = 0; d < 2; ++d) pc0[d] = s_org[d] / 2 - s_porg[d] + NG - 2;          // covers fine ghosts and the slope stencil
-    {
-      const int g = s_org[2] + k - NG;
-      pc0[2] = ((g + 64) / 2 - 32) - s_porg[2] + NG - 1;
+    for (int v = 0; v < NV; ++v) {
+      const T *po = Co + size_t(v) * Layout<T>::VS, *pn = Cn + size_t(v) * Layout<T>::VS;
+      s_par[v * CTV + r0] = only_old ? po[c0] : (only_new ? pn[c0] : (T(1) - alpha) * po[c0] + alpha * pn[c0]);
+      if (c1 >= 0) s_par[v * CTV + r1] = only_old ? po[c1] : (only_new ? pn[c1] : (T(1) - alpha) * po[c1] + alpha * pn[c1]);
     }
-    for (int t = threadIdx.x; t < NV * CTV; t += 256) {
-      const int v = t / CTV, r = t % CTV;
-      const int c = cell<T>(pc0[2] + r / (CT * CT), pc0[1] + (r / CT) % CT, pc0[0] + r % CT);
-      const T *o = Co + size_t(v) * Layout<T>::VS, *n = Cn + size_t(v) * Layout<T>::VS;
-      s_par[t] = only_old ? o[c] : (only_new ? n[c] : (T(1) - alpha) * o[c] + alpha * n[c]);
-    }
-    __syncthreads();
   }
   // ghost cells of this plane: all 400 on a z-ghost plane, else the 144 of the frame
   const int ncell = oz != 0 ? NP * NP : NP * NP - NI * NI;
-  for (int t = threadIdx.x; t < ncell; t += 256) {
-    int i, j;
+  auto locate = [&](int t, int &i, int &j) {
     if (oz != 0) { i = t % NP; j = t / NP; }
     else if (t < 2 * NG * NP) { i = t % NP; j = t / NP; if (j >= NG) j += NI; }      // rows 0,1,18,19
     else { const int u = t - 2 * NG * NP; j = NG + u / (2 * NG); i = u % (2 * NG); if (i >= NG) i += NI; }
-    const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0);
-    const int oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
-    const int r = (oz + 1) * 9 + (oy + 1) * 3 + (ox + 1);
-    const int nb = s_nbr[r];
-    const int me = cell<T>(k, j, i);
-    if (nb >= 0) {
-      if (skip_siblings) continue;
+  };
+  // sibling copies first: their loads travel with the tile's
+  if (!skip_siblings) {
+    for (int t = threadIdx.x; t < ncell; t += 256) {
+      int i, j;
+      locate(t, i, j);
+      const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
+      const int nb = nbr[(oy + 1) * 3 + (ox + 1)];
+      if (nb < 0) continue;
       const T *S = pool.patch(slot, nb);
-      const int sc = cell<T>(k - oz * NI, j - oy * NI, i - ox * NI);
+      const int me = cell<T>(k, j, i), sc = cell<T>(k - oz * NI, j - oy * NI, i - ox * NI);
 #pragma unroll
       for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + me] = S[size_t(v) * Layout<T>::VS + sc];
-    } else if (nb == -1 && Q >= 0) {
-      const int pad[3] = {i, j, k};
-      int lc[3];
-      T s[3];
+    }
+  }
+  if (!cf) return;                                   // block-uniform
+  __syncthreads();
+  for (int t = threadIdx.x; t < ncell; t += 256) {
+    int i, j;
+    locate(t, i, j);
+    const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
+    if (nbr[(oy + 1) * 3 + (ox + 1)] != -1) continue;
+    const int pad[3] = {i, j, k};
+    int c0 = 0;
+    T s[3];
+    const int st[3] = {1, CT, CT * CT};
+    const int o = octant[p];
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        const int g = s_org[d] + pad[d] - NG;        // fine global index (>= -2)
-        const int gc = (g + 64) / 2 - 32;            // floor(g/2) for g >= -64
-        s[d] = (g - 2 * gc == 0) ? T(-0.25) : T(0.25);
-        lc[d] = gc - s_porg[d] + NG - pc0[d];        // index in the staged tile
-      }
-      const int c0 = (lc[2] * CT + lc[1]) * CT + lc[0];
-      const int st[3] = {1, CT, CT * CT};
+    for (int d = 0; d < 3; ++d) {
+      const int f = pad[d] - NG;                     // fine index relative to the patch (>= -2)
+      const int fc = (f + 64) / 2 - 32;              // floor(f/2)
+      s[d] = (f - 2 * fc == 0) ? T(-0.25) : T(0.25);
+      c0 += (8 * ((o >> d) & 1) + fc + NG - pc0[d]) * st[d];
+    }
+    const int me = cell<T>(k, j, i);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const T *c = s_par + v * CTV;
-        const T uc = c[c0];
-        T val = uc;
+    for (int v = 0; v < NV; ++v) {
+      const T *c = s_par + v * CTV;
+      const T uc = c[c0];
+      T val = uc;
 #pragma unroll
-        for (int d = 0; d < 3; ++d) val = val + s[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
-        U[size_t(v) * Layout<T>::VS + me] = val;
-      }
+      for (int d = 0; d < 3; ++d) val = val + s[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
+      U[size_t(v) * Layout<T>::VS + me] = val;
     }
   }
 }
