@@ -51,7 +51,6 @@ struct amrhydro {
   std::vector<int> smax_slot;               // slot the cached value belongs to, -1 = stale
   int zsplit = 2;                           // rk_stage_march: 0 never, 1 always, 2 = levels of at most num_sms/2 patches
   int num_sms = 148;
-  int coop_reflux = 1;                      // reflux: six faces in one cooperative launch when all blocks are resident
   int fuse_cfl = 2;                         // 0 never, 1 always, 2 = where it is free (fp32)
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
@@ -595,21 +594,10 @@ int amrhydro_reflux(amrhydro_t *h, int clev, int slot) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
     const int nf = h->lev_count[clev + 1];
-    if (h->coop_reflux && nf <= 16 * h->num_sms) {            // all blocks resident: one cooperative launch, faces ordered by grid barriers
-      Pool<T> pool = make_pool<T>(h);
-      int first = h->lev_first[clev + 1];
-      const Desc *desc = h->d_desc;
-      const int *oct = h->d_octant;
-      T *Rf = (T *)h->d_Rf, *Rc = (T *)h->d_Rc, hc = T(h->dx0 / double(1 << clev));
-      void *args[] = {&pool, &slot, &first, &desc, &oct, &Rf, &Rc, &hc};
-      CUDA_TRY(h, cudaLaunchCooperativeKernel((const void *)k_reflux_all<T, NV>, dim3(nf), dim3(64), args, 0, h->stream));
-      ++h->launches;
-      return 0;
-    }
-    for (int f = 0; f < 6; ++f) {
-      k_reflux<T, NV><<<nf, 64, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[clev + 1], f,
-                                                 h->d_desc, h->d_octant, (T *)h->d_Rf, (T *)h->d_Rc,
-                                                 T(h->dx0 / double(1 << clev)));
+    for (int axis = 0; axis < 3; ++axis) {
+      k_reflux<T, NV><<<dim3(nf, 2), 64, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[clev + 1], 2 * axis,
+                                                          h->d_desc, h->d_octant, (T *)h->d_Rf, (T *)h->d_Rc,
+                                                          T(h->dx0 / double(1 << clev)));
       LAUNCH_CHECK(h);
     }
     return 0;

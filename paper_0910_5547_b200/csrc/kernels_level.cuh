@@ -2,8 +2,6 @@
 // (a2), restriction (a7), flux registers + refluxing (a8), host staging pack/unpack.
 // The paper leaves all of these on the CPU inside Enzo; readings S4-S10.
 #pragma once
-#include <cooperative_groups.h>
-
 #include "layout.cuh"
 #include "physics.cuh"
 
@@ -368,13 +366,16 @@ __global__ void __launch_bounds__(64) k_flux_registers(int first, int level, con
 }
 
 // ------------------------------------------------------------------ a8: refluxing (S10)
-// Launched once per face f = 0..5 (fixed order: a coarse cell is touched by at most one
-// fine face per launch, so there are no races and the rounding order is deterministic).
+// Launched once per axis with both faces of that axis (gridDim.y = 2), in the fixed order x, y, z: fine patches
+// cover octants of 8 coarse cells, so an uncovered coarse cell cannot touch fine patches on both sides along
+// one axis -- it is corrected by at most one face per launch (no races), and the launches keep the face order
+// f = 0..5 of S10 for the cells that get corrections along several axes (deterministic rounding).
 template <typename T, int NV>
 __global__ void __launch_bounds__(64) k_reflux(Pool<T> pool, int slot, int first_fine, int f,
                                                const Desc *__restrict__ desc, const int *__restrict__ octant,
                                                T *__restrict__ Rf, T *__restrict__ Rc, T hc) {
   const int p = first_fine + blockIdx.x;
+  f += blockIdx.y;                               // (launched per axis with gridDim.y = 2: the low and the high face)
   if (desc[p].nbr[face_region(f)] != -1) return;
   const int Q = desc[p].parent, o = octant[p];
   const int oc[3] = {o & 1, (o >> 1) & 1, (o >> 2) & 1};
@@ -400,44 +401,6 @@ __global__ void __launch_bounds__(64) k_reflux(Pool<T> pool, int slot, int first
     T *u = U + size_t(v) * Layout<T>::VS + c;
     *u = hi ? (*u + corr) : (*u - corr);
     rf[r] = T(0); rc[r] = T(0);
-  }
-}
-
-// The six faces in one cooperative launch (all blocks resident): the fixed face order of S10 is kept by a
-// grid-wide barrier between faces instead of by six launches -- same arithmetic, same order, one launch.
-template <typename T, int NV>
-__global__ void __launch_bounds__(64) k_reflux_all(Pool<T> pool, int slot, int first_fine, const Desc *__restrict__ desc,
-                                                   const int *__restrict__ octant, T *__restrict__ Rf, T *__restrict__ Rc, T hc) {
-  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
-  const int p = first_fine + blockIdx.x;
-  const int Q = desc[p].parent, o = octant[p];
-  const int oc[3] = {o & 1, (o >> 1) & 1, (o >> 2) & 1};
-  const int ca = threadIdx.x & 7, cb = threadIdx.x >> 3;
-  for (int f = 0; f < 6; ++f) {
-    if (f) grid.sync();
-    if (desc[p].nbr[face_region(f)] != -1) continue;
-    const int d = f >> 1, hi = f & 1;
-    const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;
-    int cn = NG + 8 * oc[d] + (hi ? 8 : -1);
-    int tgt = Q;
-    if (cn < NG || cn >= NG + NI) {
-      tgt = desc[Q].nbr[face_region(f)];
-      if (tgt < 0) continue;                      // improper nesting is rejected by set_hierarchy
-      cn += hi ? -NI : NI;
-    }
-    T *U = pool.patch(slot, tgt);
-    T *rf = Rf + (size_t(p) * 6 + f) * NV * 64, *rc = Rc + (size_t(p) * 6 + f) * NV * 64;
-    int pad[3];
-    pad[d] = cn; pad[d1] = NG + 8 * oc[d1] + ca; pad[d2] = NG + 8 * oc[d2] + cb;
-    const int c = cell<T>(pad[2], pad[1], pad[0]);
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      const int r = v * 64 + cb * 8 + ca;
-      const T corr = (rf[r] - rc[r]) / hc;
-      T *u = U + size_t(v) * Layout<T>::VS + c;
-      *u = hi ? (*u + corr) : (*u - corr);
-      rf[r] = T(0); rc[r] = T(0);
-    }
   }
 }
 
