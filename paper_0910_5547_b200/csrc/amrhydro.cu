@@ -16,10 +16,8 @@
 #include "layout.cuh"
 #include "physics.cuh"
 #include "rk_stage_ref.cuh"
-#include "rk_stage_tile.cuh"
 #include "rk_stage_march.cuh"
-#include "rk_stage_lite.cuh"
-#include "rk_stage_quad.cuh"
+#include "rk_stage_pair.cuh"
 
 using namespace amr;
 
@@ -55,8 +53,7 @@ struct amrhydro {
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
-  CUtensorMap tmap;            // TMA view of the pool, 16x16 boxes (rk_stage_march)
-  CUtensorMap tmap8;           // the same with 8x8 boxes (rk_stage_quad)
+  CUtensorMap tmap;            // TMA view of the pool, 16x16 boxes (rk_stage_march, rk_stage_pair)
   bool have_tmap = false;
   std::string err;
 };
@@ -198,7 +195,7 @@ int amrhydro_set_option(amrhydro_t *h, int key, double value) {
       (key == AMRHYDRO_OPT_RHO_FLOOR ? h->rho_floor : h->e_floor) = value;
       return 0;
     case AMRHYDRO_OPT_KERNEL:
-      if (value < 0 || value > 4 || value != int(value)) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0..4");
+      if (value != 0 && value != 2 && value != 3) return fail(h, AMRHYDRO_EINVAL, "kernel must be 0, 2 or 3");
       h->kernel = int(value);
       return 0;
     case AMRHYDRO_OPT_HALO:
@@ -262,8 +259,7 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   {
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      int e = make_tensor_map<T, decltype(nv)::value>(&h->tmap, dev_pool, size_t(max_patches), nslots);
-      return e ? e : make_tensor_map<T, decltype(nv)::value>(&h->tmap8, dev_pool, size_t(max_patches), nslots, 8);
+      return make_tensor_map<T, decltype(nv)::value>(&h->tmap, dev_pool, size_t(max_patches), nslots);
     });
     h->have_tmap = (r == 0);
     if (r) { h->bound = false; return fail(h, AMRHYDRO_ECUDA, "cuTensorMapEncodeTiled failed for the pool"); }
@@ -523,43 +519,30 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     const int n = h->lev_count[level], first = h->lev_first[level];
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
     smax_touch(h, level, sout);
-    if (NV == 9 && h->kernel != 0 && h->kernel != 2)
-      return fail(h, AMRHYDRO_EINVAL, "nvars = 9 runs on rk_stage kernels 0 and 2");
+    // the combination stage can also reduce the max signal speed of what it writes (a1 fused into a6)
+    const bool fuse = h->kernel != 0 && (h->fuse_cfl == 1 || (h->fuse_cfl == 2 && h->bits == 32)) && a != 0.0;
+    const int zs = (h->zsplit == 1 || (h->zsplit == 2 && 2 * n <= h->num_sms)) ? 1 : 0;
+    if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
                                                                 T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
       LAUNCH_CHECK(h);
-    } else if (h->kernel == 4) {
-      if constexpr (NV != 9) {
-        int r = launch_rk_stage_quad<T, NV>(h->tmap8, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
-        if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_quad: ") + cudaGetErrorString((cudaError_t)r));
+    } else if (h->kernel == 3 && NV == 5) {
+      if constexpr (NV == 5) {
+        int r = launch_rk_stage_pair<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
+                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
+                                            fuse ? h->d_smax + level : nullptr, zs);
+        if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_pair: ") + cudaGetErrorString((cudaError_t)r));
         LAUNCH_CHECK(h);
       }
-    } else if (h->kernel == 3) {
-      if constexpr (NV != 9) {
-        int r = launch_rk_stage_lite<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
-        if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_lite: ") + cudaGetErrorString((cudaError_t)r));
-        LAUNCH_CHECK(h);
-      }
-    } else if (h->kernel == 2) {
-      // the combination stage also reduces the max signal speed of what it writes (a1 fused into a6)
-      const bool fuse = (h->fuse_cfl == 1 || (h->fuse_cfl == 2 && h->bits == 32)) && a != 0.0;
-      if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
+    } else {
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                           fuse ? h->d_smax + level : nullptr,
-                                           (h->zsplit == 1 || (h->zsplit == 2 && 2 * n <= h->num_sms)) ? 1 : 0);
+                                           fuse ? h->d_smax + level : nullptr, zs);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
-      if (fuse) h->smax_slot[level] = sout;
-    } else if constexpr (NV != 9) {
-      int r = launch_rk_stage_tile<T, NV>(make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
-                                          make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream);
-      if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_tile: ") + cudaGetErrorString((cudaError_t)r));
-      LAUNCH_CHECK(h);
     }
+    if (fuse) h->smax_slot[level] = sout;
     if (regs) {
       k_flux_registers<T, NV><<<dim3(n, 54), 64, 0, h->stream>>>(first, level, h->d_desc, h->d_child, bflux,
                                                                   (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt));

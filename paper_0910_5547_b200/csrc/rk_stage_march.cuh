@@ -628,7 +628,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
 // origin is the first interior cell of a row, so that the global address is 32-byte aligned for
 // both element types.  Box = one interior plane of all variables of one patch.
 template <typename T, int NV>
-int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int nslots, int box_xy = NI) {
+int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int nslots) {
   typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -642,7 +642,7 @@ int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int ns
   const cuuint64_t dims[4] = {cuuint64_t(NI), cuuint64_t(NP), cuuint64_t(NP), cuuint64_t(nslots) * max_patches * NV};
   const cuuint64_t strides[3] = {cuuint64_t(Layout<T>::PX) * sizeof(T), cuuint64_t(Layout<T>::PLANE) * sizeof(T),
                                  cuuint64_t(Layout<T>::VS) * sizeof(T)};
-  const cuuint32_t box[4] = {cuuint32_t(box_xy), cuuint32_t(box_xy), 1, NV};
+  const cuuint32_t box[4] = {cuuint32_t(NI), cuuint32_t(NI), 1, NV};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   void *origin = (char *)pool_base + size_t(Layout<T>::LEAD + NG) * sizeof(T);
   CUresult r = enc(tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, origin, dims,

@@ -1,0 +1,457 @@
+// rk_stage_pair.cuh -- the hot kernel, second design: one method-of-lines stage of every 16^3 patch
+// of a level (steps a3-a6: PAPER.md:79 Eq. 7, :94-98 Eq. 8, :104-112 Eq. 9-11, :114-118 Eq. 12).
+//
+// ncu on k_rk_stage_march (rk_stage_march.cuh) showed a latency-bound kernel: one 10-warp CTA per SM,
+// 56 % of cycles with no eligible warp, 746 thread-instructions per cell of which 16 % in two halo
+// warps and 11 % in shared-memory traffic (profiles/README.md, r1).  This kernel keeps what worked
+// (z-march, TMA rings on mbarriers, every slope and face flux computed once, the arithmetic of
+// mk::prim / mk::slope4 / mk::face_flux) and changes the decomposition:
+//  * a thread owns TWO x-adjacent columns (2px, 2px+1) of row j: 128 threads (4 warps) per patch, two
+//    CTAs per SM at up to 255 registers.  The two cells give every step two independent dependency
+//    chains (ILP 2); the x face between them never leaves the registers; all own-cell and y-direction
+//    shared-memory accesses are 16-byte (fp64) / 8-byte (fp32) vectors: about half the LDS/STS
+//    instructions per cell; the update is stored with 16-byte stores.
+//  * no halo warps: each of the 128 threads also converts ONE of the 128 halo cells of a plane
+//    (loaded one plane ahead straight from the sibling's interior or the own ghost zone), and the
+//    ghost-cell slopes + the fluxes through faces 16 are two full-warp passes per plane that rotate
+//    over the four warps.
+//  * the flux arrays alias the q+ arrays (a slot is read as q+ by its only reader before that same
+//    thread overwrites it with its flux), U_base rides on a 2-slot TMA ring of its own: 91-113 kB of
+//    shared memory per CTA (fp64 Euler), so that two CTAs fit an SM in both stages.
+// Results are those of k_rk_stage_march up to the rounding of c = q_{i+1} - q_{i-1} (taken directly,
+// as the oracle does, in x and y).
+#pragma once
+#include "rk_stage_march.cuh"
+
+namespace amr {
+namespace pk {
+
+template <typename T> struct V2T;
+template <> struct V2T<double> { using type = double2; };
+template <> struct V2T<float> { using type = float2; };
+template <typename T> __device__ __forceinline__ typename V2T<T>::type ld2(const T *p) {
+  return *reinterpret_cast<const typename V2T<T>::type *>(p);
+}
+template <typename T> __device__ __forceinline__ void st2(T *p, T x, T y) {
+  typename V2T<T>::type v;
+  v.x = x; v.y = y;
+  *reinterpret_cast<typename V2T<T>::type *>(p) = v;
+}
+
+constexpr int THREADS = 128;
+
+template <typename T, int NV, bool WB> struct Smem {
+  static constexpr int NSLOT = 4;                  // ring of raw conserved planes (TMA)
+  static constexpr int BSLOT = 2;                  // ring of U_base planes (combination stage)
+  static constexpr int RAWP = NV * NI * NI;        // one raw plane [NV][16][16], dense TMA box
+  static constexpr int PW = NP;                    // primitive plane [20][20]: even pitch, pairs are 16-byte aligned
+  static constexpr int WV = NP * PW;
+  static constexpr int QXP = 9, QXV = NI * QXP;    // [16 rows][9]: slot t = q+ of cell 2t-1 / flux through face 2t
+  static constexpr int QYV = (NI + 1) * NI;        // [17][16]: slot j = q+ of row j-1 / flux through face j
+  static constexpr int HQV = 16;                   // q- of the ghost cell 16 of every line (per direction)
+  static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
+                       O_QY = ((O_QX + NV * QXV + 1) / 2) * 2, O_HQ = O_QY + NV * QYV,
+                       O_BRAW = ((O_HQ + 2 * NV * HQV + 31) / 32) * 32;
+  static constexpr int O_END = O_BRAW + (WB ? BSLOT * RAWP : 0);
+  static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
+  static constexpr size_t BYTES = BAR_OFF + (NSLOT + BSLOT) * 8 + 128;   // + slack to align the ring to 128 B
+};
+
+// limited slope in the form the update needs (fp64): returns mr and qs such that q-+ = q0 -+ qs * mr,
+// qs = 1/4 when dm and dp have the same sign bit, else 0 (one 32-bit select on the high word).
+// mr = theta2 * m1 if |theta2 * m1| < |c| else c, m1 = the smaller of dm, dp in magnitude: the value of
+// mk::slope4 (the sign of m1 and of c is that of dm whenever the signs agree).
+__device__ __forceinline__ double slope_mr(double dm, double dp, double c, double theta2, double &qs) {
+  const double m1 = fabs(dm) < fabs(dp) ? dm : dp;
+  const double t2 = theta2 * m1;
+  const double mr = fabs(t2) < fabs(c) ? t2 : c;
+  qs = __hiloint2double(((__double2hiint(dm) ^ __double2hiint(dp)) >= 0) ? 0x3fd00000 : 0, 0);
+  return mr;
+}
+__device__ __forceinline__ float slope_mr(float dm, float dp, float c, float theta2, float &qs) {
+  qs = 0.25f;
+  return mk::slope4(dm, dp, c, theta2);
+}
+
+// floors of four faces at once (S11): one integer min chain + one rarely taken branch
+template <typename T, int NV>
+__device__ __forceinline__ void floor_faces4(T (&A0)[NV], T (&B0)[NV], T (&A1)[NV], T (&B1)[NV], T (&A2)[NV], T (&B2)[NV],
+                                             T (&A3)[NV], T (&B3)[NV], const Params<T> &P, int &hits) {
+  using mk::hiw;
+  const int hr = min(min(min(hiw(A0[0]), hiw(B0[0])), min(hiw(A1[0]), hiw(B1[0]))),
+                     min(min(hiw(A2[0]), hiw(B2[0])), min(hiw(A3[0]), hiw(B3[0]))));
+  const int he = min(min(min(hiw(A0[1]), hiw(B0[1])), min(hiw(A1[1]), hiw(B1[1]))),
+                     min(min(hiw(A2[1]), hiw(B2[1])), min(hiw(A3[1]), hiw(B3[1]))));
+  if ((hr <= hiw(P.rho_floor)) | (he <= hiw(P.e_floor))) {
+    mk::floor_states<T, NV>(A0, B0, P, hits);
+    mk::floor_states<T, NV>(A1, B1, P, hits);
+    mk::floor_states<T, NV>(A2, B2, P, hits);
+    mk::floor_states<T, NV>(A3, B3, P, hits);
+  }
+}
+
+// ghost-cell slopes of one direction for one plane: lane = (line t, side).  Low side: q+ of cell -1 into
+// slot 0 of the line; high side: q- of cell 16 into the stash (its flux follows after the barrier).
+template <typename T, int NV, int D, typename S>
+__device__ __forceinline__ void halo_slopes(T *sm, int buf, int lane, T th2) {
+  constexpr int PW = S::PW, WV = S::WV;
+  constexpr int rst = D == 0 ? 1 : PW;
+  const int t = lane & 15, hi = lane >> 4;
+  const T *s3 = sm + S::O_W + buf * (NV * WV) +
+                (D == 0 ? (t + NG) * PW + (hi ? NG + NI - 1 : 0) : (hi ? NG + NI - 1 : 0) * PW + (t + NG));
+  T *qlo = sm + (D == 0 ? S::O_QX + t * S::QXP : S::O_QY + t);
+  T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
+  constexpr int qv = D == 0 ? S::QXV : S::QYV;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const T w0 = s3[v * WV], w1 = s3[v * WV + rst], w2 = s3[v * WV + 2 * rst];
+    T qs;
+    const T mr = slope_mr(w1 - w0, w2 - w1, w2 - w0, th2, qs);
+    if (hi) hq[v * S::HQV] = fma(-qs, mr, w1);
+    else qlo[v * qv] = fma(qs, mr, w1);
+  }
+}
+// flux through face 16 of every line (lanes 0-15), after the q+ of cell 15 has been published
+template <typename T, int NV, int D, typename S>
+__device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface, int &hits) {
+  if (lane >= 16) return;
+  const int t = lane;
+  constexpr int qv = D == 0 ? S::QXV : S::QYV;
+  T *q16 = sm + (D == 0 ? S::O_QX + t * S::QXP + 8 : S::O_QY + NI * NI + t);
+  const T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
+  T WL[NV], WR[NV], G[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) { WL[v] = q16[v * qv]; WR[v] = hq[v * S::HQV]; }
+  mk::floor_states<T, NV>(WL, WR, P, hits);
+  mk::face_flux<T, D>(WL, WR, P, G);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) q16[v * qv] = G[v];
+  if (bflux) {
+    T *B = bflux + ((size_t(pl) * 9 + 3 * D + 2) * NV) * 256 + zface * 16 + t;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
+  }
+}
+
+}  // namespace pk
+
+template <typename T, int NV, bool BASE>
+__global__ void __launch_bounds__(pk::THREADS, 2)
+k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
+                T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
+                const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit) {
+  using S = pk::Smem<T, NV, BASE>;
+  constexpr int PW = S::PW, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP, NSLOT = S::NSLOT;
+  constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
+  extern __shared__ unsigned char smem_raw[];
+  T *sm = reinterpret_cast<T *>(smem_raw + ((128u - (mk::smem_u32(smem_raw) & 127u)) & 127u));   // TMA destination: 128-byte aligned
+  unsigned long long *bars = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(sm) + S::BAR_OFF);
+  unsigned long long *bbars = bars + NSLOT;
+
+  // zsplit = 1 (levels too small to fill the machine): two CTAs per patch, each marching over 8 of the 16 cells in z
+  const int pl = blockIdx.x >> zsplit, p = first + pl;
+  const int zlo = int(blockIdx.x & zsplit) * (NI / 2), nz = zsplit ? NI / 2 : NI;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = tid >> 3, px = tid & 7, i0 = 2 * px;
+  const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
+  const T th2 = T(2) * P.theta;
+  int hits = 0;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NSLOT + S::BSLOT; ++s) mk::mbar_init(&bars[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const Desc &D = desc[p];
+  // ---- this thread's halo cell: threads 0-63 the x-ghosts (row, cell -2,-1,16,17), 64-127 the y-ghosts (column, row ...)
+  const T *hsrc;
+  T *hdst;
+  {
+    int hrow, hcol, face;
+    if (tid < 64) { const int q = tid & 3; hrow = (tid >> 2) + NG; hcol = q < 2 ? q : NI + q; face = q < 2 ? 0 : 1; }
+    else { const int u = tid - 64, q = u >> 4; hcol = (u & 15) + NG; hrow = q < 2 ? q : NI + q; face = q < 2 ? 2 : 3; }
+    hdst = sm + S::O_W + hrow * PW + hcol;
+    const int nb = direct_halo ? D.nbr[face_region(face)] : -1;
+    if (nb >= 0) {                        // the sibling's interior instead of the own ghost zone
+      const int sh = (face & 1) ? -NI : NI;
+      if (face < 2) hcol += sh; else hrow += sh;
+    }
+    hsrc = pool.patch(sin, nb >= 0 ? nb : p) + LEAD + hrow * PX + hcol;
+  }
+  // ---- TMA producer state (thread 0)
+  int q_mid = 0, q_lo = 0, q_hi = 0, kz_lo = 0, kz_hi = 0, q_base = 0;
+  if (tid == 0) {
+    const int nzl = direct_halo ? D.nbr[face_region(4)] : -1, nzh = direct_halo ? D.nbr[face_region(5)] : -1;
+    const int qb = sin * pool.max_patches;
+    q_mid = (qb + p) * NV; q_lo = (qb + (nzl >= 0 ? nzl : p)) * NV; q_hi = (qb + (nzh >= 0 ? nzh : p)) * NV;
+    kz_lo = nzl >= 0 ? NI : 0; kz_hi = nzh >= 0 ? -NI : 0;
+    q_base = (sbase * pool.max_patches + p) * NV;
+  }
+  auto issue = [&](int pk_) {                                 // raw conserved interior box of padded plane pk_ of this march
+    const int slot = pk_ % NSLOT, ap = pk_ + zlo;
+    const int q = ap < NG ? q_lo : (ap >= NG + NI ? q_hi : q_mid);
+    const int k = ap < NG ? ap + kz_lo : (ap >= NG + NI ? ap + kz_hi : ap);
+    mk::mbar_expect_tx(&bars[slot], unsigned(RAWP * sizeof(T)));
+    mk::tma_load_4d(sm + S::O_RAW + slot * RAWP, &tmap, 0, NG, k, q, &bars[slot]);
+  };
+  auto issue_base = [&](int c_) {                             // U_base of cell plane c_ (Eq. 8)
+    const int slot = c_ & 1;
+    mk::mbar_expect_tx(&bbars[slot], unsigned(RAWP * sizeof(T)));
+    mk::tma_load_4d(sm + S::O_BRAW + slot * RAWP, &tmap, 0, NG, c_ + zlo, q_base, &bbars[slot]);
+  };
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) issue(s);
+    if (BASE) issue_base(NG);
+  }
+
+  const int off = LEAD + (j + NG) * PX + (i0 + NG);          // in-plane offset of this pair of columns (16-byte aligned)
+  T *out = pool.patch(sout, p) + off;
+  const T *raw = sm + S::O_RAW + j * NI + i0;                 // this pair in ring slot 0, v = 0
+  T *wme = sm + S::O_W + (j + NG) * PW + (i0 + NG);           // this pair in primitive buffer 0, v = 0
+  T *qx = sm + S::O_QX + j * S::QXP + px;                     // slot px: q+ of cell i0-1 / flux through face i0
+  T *qy = sm + S::O_QY + j * NI + i0;                         // slot j: q+ of row j-1 / flux through face j
+
+  T Uh[NV];                                                   // halo cell of the next plane to convert
+  auto halo_load = [&](int pk_) {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Uh[v] = hsrc[size_t(v) * VS + (pk_ + zlo) * PLANE];
+  };
+  auto halo_publish = [&](int pk_) {
+    T Wh[NV];
+    mk::prim<T, NV>(Uh, Wh, P, hits);
+    T *d = hdst + (pk_ & 1) * (NV * WV);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) d[v * WV] = Wh[v];
+  };
+  halo_load(NG);
+
+  T Wc[2][NV], dzm[2][NV], qpz[2][NV], acc[2][NV];
+  T best = T(0);                      // fused CFL reduction (a1) over the cells this thread finishes
+  bool bad = false;
+  {
+    T U0[2][NV], U1[2][NV], U2[2][NV], W0[2][NV], W1[2][NV];
+    mk::mbar_wait(&bars[0], 0);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + v * (NI * NI)); U0[0][v] = x.x; U0[1][v] = x.y; }
+    mk::mbar_wait(&bars[1], 0);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + RAWP + v * (NI * NI)); U1[0][v] = x.x; U1[1][v] = x.y; }
+    mk::mbar_wait(&bars[2], 0);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + 2 * RAWP + v * (NI * NI)); U2[0][v] = x.x; U2[1][v] = x.y; }
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      mk::prim<T, NV>(U0[s], W0[s], P, hits);
+      mk::prim<T, NV>(U1[s], W1[s], P, hits);
+      mk::prim<T, NV>(U2[s], Wc[s], P, hits);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const T dm = W1[s][v] - W0[s][v];
+        dzm[s][v] = Wc[s][v] - W1[s][v];
+        T qs;
+        const T mr = pk::slope_mr(dm, dzm[s][v], dm + dzm[s][v], th2, qs);
+        qpz[s][v] = fma(qs, mr, W1[s][v]);                       // q+ of the ghost cell below plane 2
+        acc[s][v] = T(0);
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) pk::st2(wme + v * WV, Wc[0][v], Wc[1][v]);   // plane 2 -> primitive buffer 0
+  }
+  halo_publish(NG);
+  if (nz > 1) halo_load(NG + 1);
+  __syncthreads();
+  if (tid == 0) issue(NSLOT);                                 // slot of plane 0: converted, never needed again
+
+#pragma unroll 1
+  for (int c = NG; c <= NG + nz; ++c) {            // current cell = plane c of this march (2..nz+1); c = nz+2: last z face only
+    const bool live = c < NG + nz;                 // plane c is a cell of this march
+    // 1. plane c+1: raw -> primitives, published for the x/y neighbours; this thread's halo cell of that plane
+    T Wn[2][NV];
+    {
+      const int slot = (c + 1) % NSLOT;
+      mk::mbar_wait(&bars[slot], unsigned((c + 1) / NSLOT) & 1u);
+      T Un[2][NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + slot * RAWP + v * (NI * NI)); Un[0][v] = x.x; Un[1][v] = x.y; }
+      mk::prim<T, NV>(Un[0], Wn[0], P, hits);
+      mk::prim<T, NV>(Un[1], Wn[1], P, hits);
+    }
+    if (c + 1 < NG + nz) {
+      T *w = wme + ((c + 1) & 1) * (NV * WV);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) pk::st2(w + v * WV, Wn[0][v], Wn[1][v]);
+      halo_publish(c + 1);
+      if (c + 2 < NG + nz) halo_load(c + 2);
+    }
+    // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
+    {
+      T Gz[2][NV], qm[2][NV];
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const T dp = Wn[s][v] - Wc[s][v];
+          T qs;
+          const T mr = pk::slope_mr(dzm[s][v], dp, dzm[s][v] + dp, th2, qs);
+          qm[s][v] = fma(-qs, mr, Wc[s][v]);
+          dzm[s][v] = dp;
+          Gz[s][v] = fma(qs, mr, Wc[s][v]);                        // q+ of cell c, parked until qpz has been used
+        }
+      {
+        T L0[NV], L1[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { L0[v] = qpz[0][v]; L1[v] = qpz[1][v]; qpz[0][v] = Gz[0][v]; qpz[1][v] = Gz[1][v]; }
+        mk::floor_states2<T, NV>(L0, qm[0], L1, qm[1], P, hits);
+        mk::face_flux<T, 2>(L0, qm[0], P, Gz[0]);
+        mk::face_flux<T, 2>(L1, qm[1], P, Gz[1]);
+      }
+      if (bflux && ((c - NG + zlo) & 7) == 0) {
+        T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG + zlo) >> 3)) * NV) * 256 + j * 16 + i0;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gz[0][v], T(0.5) * Gz[1][v]);
+      }
+      if (c > NG) {
+        const T *ui = raw + ((c - 1) % NSLOT) * RAWP;        // raw U of cell c-1 is still in the ring
+        const T *ub = raw + (S::O_BRAW - S::O_RAW) + ((c - 1) & 1) * RAWP;
+        if (BASE) mk::mbar_wait(&bbars[(c - 1) & 1], unsigned((c - 1 - NG) >> 1) & 1u);
+        T *o = out + (c - 1 + zlo) * PLANE;
+        T un[2][NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const auto x = pk::ld2(ui + v * (NI * NI));
+          T pre0 = b * x.x, pre1 = b * x.y;
+          if (BASE) {
+            const auto y = pk::ld2(ub + v * (NI * NI));
+            pre0 = fma(a, y.x, pre0); pre1 = fma(a, y.y, pre1);
+          }
+          un[0][v] = fma(-kk, acc[0][v] + Gz[0][v], pre0);          // Eq. 7-8
+          un[1][v] = fma(-kk, acc[1][v] + Gz[1][v], pre1);
+          pk::st2(o + size_t(v) * VS, un[0][v], un[1][v]);
+        }
+        if (BASE && smax_out) {
+          // S4 on the state just produced: max_d |v_d| + c_d, with the NaN/inf test of k_cfl
+#pragma unroll
+          for (int s = 0; s < 2; ++s) {
+            T Wq[NV];
+            mk::prim<T, NV>(un[s], Wq, P, hits);
+            const T sp = mk::max_speed_fast<T, NV>(Wq, P);
+            const T chk = ((Wq[2] + Wq[3]) + Wq[4]) + sp;
+            bad |= !(chk - chk == T(0));
+            best = tmax(best, sp);
+          }
+        }
+      }
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { acc[0][v] = -Gz[0][v]; acc[1][v] = -Gz[1][v]; }   // the low z face enters with its sign
+    }
+    if (live) {
+      // 3. x/y phase 1: slopes of both cells along x and y, publish the q+ the neighbours need
+      const T *w = wme + (c & 1) * (NV * WV);
+      T qmx0[NV], qpx0[NV], qmx1[NV], qmy0[NV], qmy1[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const T a0 = Wc[0][v], a1 = Wc[1][v];
+        const T wl = w[v * WV - 1], wr = w[v * WV + 2];
+        const auto wd = pk::ld2(w + v * WV - PW), wu = pk::ld2(w + v * WV + PW);
+        const T d0 = a0 - wl, d1 = a1 - a0, d2 = wr - a1;
+        T qs, mr;
+        mr = pk::slope_mr(d0, d1, a1 - wl, th2, qs);
+        qmx0[v] = fma(-qs, mr, a0); qpx0[v] = fma(qs, mr, a0);
+        mr = pk::slope_mr(d1, d2, wr - a0, th2, qs);
+        qmx1[v] = fma(-qs, mr, a1);
+        qx[v * QXV + 1] = fma(qs, mr, a1);
+        mr = pk::slope_mr(a0 - wd.x, wu.x - a0, wu.x - wd.x, th2, qs);
+        qmy0[v] = fma(-qs, mr, a0);
+        const T qpy0 = fma(qs, mr, a0);
+        mr = pk::slope_mr(a1 - wd.y, wu.y - a1, wu.y - wd.y, th2, qs);
+        qmy1[v] = fma(-qs, mr, a1);
+        pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
+      }
+      if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
+      if (warp == ((c + 2) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
+      __syncthreads();
+      if (tid == 0) {                              // ring slots that nobody reads any more
+        if (c + NSLOT - 1 < nz + 2 * NG) issue(c + NSLOT - 1);          // slot of plane c-1: cell c-1 is finished
+        if (BASE && c + 1 < NG + nz) issue_base(c + 1);                 // slot of cell c-1
+      }
+      // 4. phase 2: fluxes through the low x and y faces of both cells
+      T Gx0[NV], Gx1[NV], Gy0[NV], Gy1[NV];
+      {
+        T WL[NV], WD0[NV], WD1[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          WL[v] = qx[v * QXV];
+          const auto y = pk::ld2(qy + v * QYV);
+          WD0[v] = y.x; WD1[v] = y.y;
+        }
+        pk::floor_faces4<T, NV>(WL, qmx0, qpx0, qmx1, WD0, qmy0, WD1, qmy1, P, hits);
+        mk::face_flux<T, 0>(WL, qmx0, P, Gx0);
+        mk::face_flux<T, 0>(qpx0, qmx1, P, Gx1);
+        mk::face_flux<T, 1>(WD0, qmy0, P, Gy0);
+        mk::face_flux<T, 1>(WD1, qmy1, P, Gy1);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { qx[v * QXV] = Gx0[v]; pk::st2(qy + v * QYV, Gy0[v], Gy1[v]); }
+      }
+      if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo, hits);
+      if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo, hits);
+      if (bflux) {
+        if ((i0 & 7) == 0) {
+          T *B = bflux + ((size_t(pl) * 9 + 0 + (i0 >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + j;
+#pragma unroll
+          for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx0[v];
+        }
+        if ((j & 7) == 0) {
+          T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + i0;
+#pragma unroll
+          for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gy0[v], T(0.5) * Gy1[v]);
+        }
+      }
+      __syncthreads();
+      // 5. phase 3: flux differences in x and y (the low z face is already in acc)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const T fxh = qx[v * QXV + 1];
+        const auto fyh = pk::ld2(qy + v * QYV + NI);
+        acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) + acc[0][v];
+        acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) + acc[1][v];
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { Wc[0][v] = Wn[0][v]; Wc[1][v] = Wn[1][v]; }
+  }
+  if (BASE && smax_out) {
+    // one atomicMax per warp on the bit pattern of a non-negative double (monotone as an unsigned integer)
+    double bq = bad ? __longlong_as_double(0x7ff0000000000000LL) : double(best);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bq = fmax(bq, __shfl_xor_sync(0xffffffffu, bq, o));
+    if (lane == 0) atomicMax(smax_out, (unsigned long long)__double_as_longlong(bq));
+  }
+  if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
+}
+
+// returns 0 or a cudaError_t
+template <typename T, int NV>
+int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
+                         T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
+                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0) {
+  static bool configured = false;
+  constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES, bytes1 = pk::Smem<T, NV, true>::BYTES;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_rk_stage_pair<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(k_rk_stage_pair<T, NV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes1));
+    if (e != cudaSuccess) return int(e);
+    configured = true;
+  }
+  if (a != T(0))
+    k_rk_stage_pair<T, NV, true><<<n << zsplit, pk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                              bflux, floor_hits, desc, direct_halo, smax_out, zsplit);
+  else
+    k_rk_stage_pair<T, NV, false><<<n << zsplit, pk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                               bflux, floor_hits, desc, direct_halo, nullptr, zsplit);
+  return 0;
+}
+
+}  // namespace amr

@@ -157,10 +157,8 @@ def test_fill_ghosts_prolongation_matches_oracle(gpu, kind, alpha):
 # ------------------------------------------------------------------ a3-a6: one stage
 @pytest.mark.parametrize("nv", [5, 8, 9])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("kernel,halo", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1), (4, 0), (4, 1)])
+@pytest.mark.parametrize("kernel,halo", [(0, 0), (2, 0), (2, 1), (3, 0), (3, 1)])
 def test_rk_stage_matches_oracle(gpu, nv, dtype, kernel, halo):
-    if nv == 9 and kernel not in (0, 2):
-        pytest.skip("the 9-variable system runs on the reference and the default stage kernel")
     h = wl.uniform_hierarchy(2, periodic=True)
     g, o = make_pair(gpu, h, 5.0 / 3.0, nv, dtype, kernel=kernel, halo=halo, ch=1.7)
     upload_both(g, o, rand_state(h, nv, 6, 5.0 / 3.0), dtype)
@@ -185,7 +183,7 @@ def test_rk_stage_theta_option(gpu, theta):
     assert norm_err(g.download(1), o.download(1)).max() <= 1e-13
 
 
-@pytest.mark.parametrize("kernel,halo", [(0, 0), (2, 0), (2, 1), (3, 1), (4, 1)])
+@pytest.mark.parametrize("kernel,halo", [(0, 0), (2, 0), (2, 1), (3, 0), (3, 1)])
 def test_rk_stage_with_active_floors(gpu, kernel, halo):
     """S11 as a degenerate case: floors set inside the range of the data, so that they fire in the
     primitive recovery and on reconstructed states; values must still agree with the oracle."""
@@ -230,20 +228,16 @@ def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
     h = wl.uniform_hierarchy(2, periodic=False)
     U = rand_state(h, 5, 8)
     res = []
-    for kernel, halo in ((0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1), (4, 0), (4, 1)):
+    for kernel, halo in ((0, 0), (2, 0), (2, 1), (3, 0), (3, 1)):
         g = gpu.AmrHydro(h, 1.4, 5, kernel=kernel, halo=halo)
         g.upload(0, U)
         g.fill_ghosts(0, 0)
         g.rk_stage(0, 0, 0, 1, 0.0, 1.0, 1e-3)
         res.append(g.download(1))
     assert norm_err(res[1], res[0]).max() <= 1e-14
-    assert norm_err(res[3], res[0]).max() <= 1e-14
     assert np.array_equal(res[1], res[2])      # halo source does not change the arithmetic
+    assert norm_err(res[3], res[0]).max() <= 1e-14
     assert np.array_equal(res[3], res[4])
-    assert norm_err(res[5], res[0]).max() <= 1e-14
-    assert np.array_equal(res[5], res[6])
-    assert norm_err(res[7], res[0]).max() <= 1e-14
-    assert np.array_equal(res[7], res[8])
 
 
 def test_uniform_state_bitwise_on_gpu(gpu):
