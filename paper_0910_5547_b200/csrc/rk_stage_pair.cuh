@@ -54,18 +54,21 @@ template <typename T, int NV, bool WB> struct Smem {
                        O_BRAW = ((O_HQ + 2 * NV * HQV + 31) / 32) * 32;
   static constexpr int O_END = O_BRAW + (WB ? BSLOT * RAWP : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
-  static constexpr size_t BYTES = BAR_OFF + (NSLOT + BSLOT) * 8 + 128;   // + slack to align the ring to 128 B
+  static constexpr size_t BYTES = BAR_OFF + (NSLOT + BSLOT + 2) * 8 + 128;   // + slack to align the ring to 128 B
 };
 
-// limited slope in the form the update needs (fp64): returns mr and qs such that q-+ = q0 -+ qs * mr,
-// qs = 1/4 when dm and dp have the same sign bit, else 0 (one 32-bit select on the high word).
-// mr = theta2 * m1 if |theta2 * m1| < |c| else c, m1 = the smaller of dm, dp in magnitude: the value of
-// mk::slope4 (the sign of m1 and of c is that of dm whenever the signs agree).
+// limited slope times 4 (fp64): mr = theta2 * m1 if |theta2 * m1| < |c| else c, m1 = the smaller of dm, dp in magnitude, and 0
+// when dm and dp differ in sign: the value of mk::slope4 (the sign of m1 and of c is that of dm whenever the signs agree).
+// The sign test is one LOP3 with a predicate result; q-+ = q0 -+ qs * mr with the constant qs = 1/4.
 __device__ __forceinline__ double slope_mr(double dm, double dp, double c, double theta2, double &qs) {
   const double m1 = fabs(dm) < fabs(dp) ? dm : dp;
   const double t2 = theta2 * m1;
-  const double mr = fabs(t2) < fabs(c) ? t2 : c;
-  qs = __hiloint2double(((__double2hiint(dm) ^ __double2hiint(dp)) >= 0) ? 0x3fd00000 : 0, 0);
+  double mr = fabs(t2) < fabs(c) ? t2 : c;
+  int differ;
+  asm("{\n .reg .pred p;\n .reg .b32 t;\n lop3.or.b32 t|p, %1, %2, 0x80000000, 0x28, 0;\n selp.b32 %0, 1, 0, p;\n}"
+      : "=r"(differ) : "r"(__double2hiint(dm)), "r"(__double2hiint(dp)));
+  if (differ) mr = 0.0;
+  qs = 0.25;
   return mr;
 }
 __device__ __forceinline__ float slope_mr(float dm, float dp, float c, float theta2, float &qs) {
@@ -73,22 +76,43 @@ __device__ __forceinline__ float slope_mr(float dm, float dp, float c, float the
   return mk::slope4(dm, dp, c, theta2);
 }
 
-// floors of four faces at once (S11): one integer min chain + one rarely taken branch
+// O1 for several cells with ONE rarely taken branch (S11): primitives without floors first, the floors of mk::prim only
+// when a density or an internal energy is at or below its floor's high word.
 template <typename T, int NV>
-__device__ __forceinline__ void floor_faces4(T (&A0)[NV], T (&B0)[NV], T (&A1)[NV], T (&B1)[NV], T (&A2)[NV], T (&B2)[NV],
-                                             T (&A3)[NV], T (&B3)[NV], const Params<T> &P, int &hits) {
+__device__ __forceinline__ void prim_nofloor(const T (&U)[NV], T (&W)[NV]) {
+  const T rho = U[0];
+  const T ir = mk::frcp(rho);
+  const T vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
+  T et = U[4];
+  if (NV >= 8) {
+    et = fma(T(-0.5), fma(U[7 % NV], U[7 % NV], fma(U[6 % NV], U[6 % NV], U[5 % NV] * U[5 % NV])), et);
+    W[5 % NV] = U[5 % NV]; W[6 % NV] = U[6 % NV]; W[7 % NV] = U[7 % NV];
+  }
+  if (NV == 9) W[8 % NV] = U[8 % NV];
+  W[0] = rho; W[1] = fma(T(-0.5), fma(vz, vz, fma(vy, vy, vx * vx)), et * ir); W[2] = vx; W[3] = vy; W[4] = vz;
+}
+template <typename T, int NV>
+__device__ __forceinline__ void prim3(const T (&Ua)[NV], const T (&Ub)[NV], const T (&Uc)[NV], bool with_c, T (&Wa)[NV],
+                                      T (&Wb)[NV], T (&Wc)[NV], const Params<T> &P, int &hits) {
   using mk::hiw;
-  const int hr = min(min(min(hiw(A0[0]), hiw(B0[0])), min(hiw(A1[0]), hiw(B1[0]))),
-                     min(min(hiw(A2[0]), hiw(B2[0])), min(hiw(A3[0]), hiw(B3[0]))));
-  const int he = min(min(min(hiw(A0[1]), hiw(B0[1])), min(hiw(A1[1]), hiw(B1[1]))),
-                     min(min(hiw(A2[1]), hiw(B2[1])), min(hiw(A3[1]), hiw(B3[1]))));
+  prim_nofloor<T, NV>(Ua, Wa);
+  prim_nofloor<T, NV>(Ub, Wb);
+  int hr = min(hiw(Wa[0]), hiw(Wb[0])), he = min(hiw(Wa[1]), hiw(Wb[1]));
+  if (with_c) {
+    prim_nofloor<T, NV>(Uc, Wc);
+    hr = min(hr, hiw(Wc[0])); he = min(he, hiw(Wc[1]));
+  }
   if ((hr <= hiw(P.rho_floor)) | (he <= hiw(P.e_floor))) {
-    mk::floor_states<T, NV>(A0, B0, P, hits);
-    mk::floor_states<T, NV>(A1, B1, P, hits);
-    mk::floor_states<T, NV>(A2, B2, P, hits);
-    mk::floor_states<T, NV>(A3, B3, P, hits);
+    mk::prim<T, NV>(Ua, Wa, P, hits);
+    mk::prim<T, NV>(Ub, Wb, P, hits);
+    if (with_c) mk::prim<T, NV>(Uc, Wc, P, hits);
   }
 }
+
+// S11 on reconstructed states: with the limiter of Eq. 9-11 and theta <= 2 a reconstructed density or internal energy
+// lies between the values of the cell and of its neighbours (|slope/2| <= theta/2 min(|dm|, |dp|)), and those have
+// been floored in the primitive recovery: the floors on l and r states cannot fire beyond one rounding of the floor
+// itself, so this kernel does not test them (k_rk_stage_march and the oracle do, S11).
 
 // ghost-cell slopes of one direction for one plane: lane = (line t, side).  Low side: q+ of cell -1 into
 // slot 0 of the line; high side: q- of cell 16 into the stash (its flux follows after the barrier).
@@ -113,7 +137,7 @@ __device__ __forceinline__ void halo_slopes(T *sm, int buf, int lane, T th2) {
 }
 // flux through face 16 of every line (lanes 0-15), after the q+ of cell 15 has been published
 template <typename T, int NV, int D, typename S>
-__device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface, int &hits) {
+__device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface) {
   if (lane >= 16) return;
   const int t = lane;
   constexpr int qv = D == 0 ? S::QXV : S::QYV;
@@ -122,7 +146,6 @@ __device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T
   T WL[NV], WR[NV], G[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) { WL[v] = q16[v * qv]; WR[v] = hq[v * S::HQV]; }
-  mk::floor_states<T, NV>(WL, WR, P, hits);
   mk::face_flux<T, D>(WL, WR, P, G);
 #pragma unroll
   for (int v = 0; v < NV; ++v) q16[v * qv] = G[v];
@@ -146,12 +169,14 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   extern __shared__ unsigned char smem_raw[];
   T *sm = reinterpret_cast<T *>(smem_raw + ((128u - (mk::smem_u32(smem_raw) & 127u)) & 127u));   // TMA destination: 128-byte aligned
   unsigned long long *bars = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(sm) + S::BAR_OFF);
-  unsigned long long *bbars = bars + NSLOT;
+  unsigned long long *bbars = bars + NSLOT;                   // U_base ring
+  unsigned long long *xbar = bbars + S::BSLOT;                // [0]: q+ published (B1), [1]: fluxes published (B2)
 
   // zsplit = 1 (levels too small to fill the machine): two CTAs per patch, each marching over 8 of the 16 cells in z
   const int pl = blockIdx.x >> zsplit, p = first + pl;
   const int zlo = int(blockIdx.x & zsplit) * (NI / 2), nz = zsplit ? NI / 2 : NI;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // (through a shuffle: the compiler then knows it is warp-uniform)
   const int j = tid >> 3, px = tid & 7, i0 = 2 * px;
   const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
   const T th2 = T(2) * P.theta;
@@ -160,6 +185,8 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < NSLOT + S::BSLOT; ++s) mk::mbar_init(&bars[s], 1);
+    mk::mbar_init(&xbar[0], pk::THREADS / 32);
+    mk::mbar_init(&xbar[1], pk::THREADS / 32);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const Desc &D = desc[p];
@@ -218,92 +245,125 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 #pragma unroll
     for (int v = 0; v < NV; ++v) Uh[v] = hsrc[size_t(v) * VS + (pk_ + zlo) * PLANE];
   };
-  auto halo_publish = [&](int pk_) {
-    T Wh[NV];
-    mk::prim<T, NV>(Uh, Wh, P, hits);
-    T *d = hdst + (pk_ & 1) * (NV * WV);
+  // raw plane pk_ -> primitives of this pair in primitive buffer pk_ & 1; with_halo: also this thread's halo cell (Uh)
+  auto convert = [&](int pk_, bool with_halo, T (&W0)[NV], T (&W1)[NV]) {
+    const int slot = pk_ % NSLOT;
+    mk::mbar_wait(&bars[slot], unsigned(pk_ / NSLOT) & 1u);
+    T U0[NV], U1[NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) d[v * WV] = Wh[v];
+    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + slot * RAWP + v * (NI * NI)); U0[v] = x.x; U1[v] = x.y; }
+    T Wh[NV];
+    pk::prim3<T, NV>(U0, U1, Uh, with_halo, W0, W1, Wh, P, hits);
+    T *w = wme + (pk_ & 1) * (NV * WV);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) pk::st2(w + v * WV, W0[v], W1[v]);
+    if (with_halo) {
+      T *d = hdst + (pk_ & 1) * (NV * WV);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) d[v * WV] = Wh[v];
+    }
   };
-  halo_load(NG);
+  // CTA barrier in two halves on an mbarrier: arrive (one lane per warp, after the warp's writes) ... wait
+  auto arrive = [&](int which) {
+    __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mk::smem_u32(&xbar[which])) : "memory");
+  };
 
-  T Wc[2][NV], dzm[2][NV], qpz[2][NV], acc[2][NV];
+  T dzm[2][NV], qpz[2][NV], acc[2][NV];
   T best = T(0);                      // fused CFL reduction (a1) over the cells this thread finishes
   bool bad = false;
+  halo_load(NG);
   {
-    T U0[2][NV], U1[2][NV], U2[2][NV], W0[2][NV], W1[2][NV];
-    mk::mbar_wait(&bars[0], 0);
+    // planes 0, 1: only the z stencil of this pair needs them; planes 2 and 3 are published
+    T W0[2][NV], W1[2][NV], W2[2][NV], W3[2][NV];
+    {
+      T U0[2][NV], U1[2][NV];
+      mk::mbar_wait(&bars[0], 0);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + v * (NI * NI)); U0[0][v] = x.x; U0[1][v] = x.y; }
-    mk::mbar_wait(&bars[1], 0);
+      for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + v * (NI * NI)); U0[0][v] = x.x; U0[1][v] = x.y; }
+      mk::mbar_wait(&bars[1], 0);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + RAWP + v * (NI * NI)); U1[0][v] = x.x; U1[1][v] = x.y; }
-    mk::mbar_wait(&bars[2], 0);
+      for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + RAWP + v * (NI * NI)); U1[0][v] = x.x; U1[1][v] = x.y; }
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + 2 * RAWP + v * (NI * NI)); U2[0][v] = x.x; U2[1][v] = x.y; }
+      for (int s = 0; s < 2; ++s) { mk::prim<T, NV>(U0[s], W0[s], P, hits); mk::prim<T, NV>(U1[s], W1[s], P, hits); }
+    }
+    convert(NG, true, W2[0], W2[1]);
+    if (nz > 1) halo_load(NG + 1);
+    convert(NG + 1, nz > 1, W3[0], W3[1]);
+    if (nz > 2) halo_load(NG + 2);
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      mk::prim<T, NV>(U0[s], W0[s], P, hits);
-      mk::prim<T, NV>(U1[s], W1[s], P, hits);
-      mk::prim<T, NV>(U2[s], Wc[s], P, hits);
+    for (int s = 0; s < 2; ++s)
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
         const T dm = W1[s][v] - W0[s][v];
-        dzm[s][v] = Wc[s][v] - W1[s][v];
+        dzm[s][v] = W2[s][v] - W1[s][v];
         T qs;
         const T mr = pk::slope_mr(dm, dzm[s][v], dm + dzm[s][v], th2, qs);
         qpz[s][v] = fma(qs, mr, W1[s][v]);                       // q+ of the ghost cell below plane 2
         acc[s][v] = T(0);
       }
-    }
-#pragma unroll
-    for (int v = 0; v < NV; ++v) pk::st2(wme + v * WV, Wc[0][v], Wc[1][v]);   // plane 2 -> primitive buffer 0
   }
-  halo_publish(NG);
-  if (nz > 1) halo_load(NG + 1);
   __syncthreads();
   if (tid == 0) issue(NSLOT);                                 // slot of plane 0: converted, never needed again
 
 #pragma unroll 1
   for (int c = NG; c <= NG + nz; ++c) {            // current cell = plane c of this march (2..nz+1); c = nz+2: last z face only
     const bool live = c < NG + nz;                 // plane c is a cell of this march
-    // 1. plane c+1: raw -> primitives, published for the x/y neighbours; this thread's halo cell of that plane
-    T Wn[2][NV];
-    {
-      const int slot = (c + 1) % NSLOT;
-      mk::mbar_wait(&bars[slot], unsigned((c + 1) / NSLOT) & 1u);
-      T Un[2][NV];
+    const unsigned par = unsigned(c - NG) & 1u;    // phase of the two exchange barriers
+    const T *w = wme + (c & 1) * (NV * WV);
+    T Wc[2][NV];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(raw + slot * RAWP + v * (NI * NI)); Un[0][v] = x.x; Un[1][v] = x.y; }
-      mk::prim<T, NV>(Un[0], Wn[0], P, hits);
-      mk::prim<T, NV>(Un[1], Wn[1], P, hits);
-    }
-    if (c + 1 < NG + nz) {
-      T *w = wme + ((c + 1) & 1) * (NV * WV);
+    for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(w + v * WV); Wc[0][v] = x.x; Wc[1][v] = x.y; }
+    T qmx0[NV], qpx0[NV], qmx1[NV], qmy0[NV], qmy1[NV];
+    if (live) {
+      // 1. slopes of both cells along x and y; publish the q+ the neighbours need
 #pragma unroll
-      for (int v = 0; v < NV; ++v) pk::st2(w + v * WV, Wn[0][v], Wn[1][v]);
-      halo_publish(c + 1);
-      if (c + 2 < NG + nz) halo_load(c + 2);
+      for (int v = 0; v < NV; ++v) {
+        const T a0 = Wc[0][v], a1 = Wc[1][v];
+        const T wl = w[v * WV - 1], wr = w[v * WV + 2];
+        const auto wd = pk::ld2(w + v * WV - PW), wu = pk::ld2(w + v * WV + PW);
+        const T d0 = a0 - wl, d1 = a1 - a0, d2 = wr - a1;
+        T qs, mr;
+        mr = pk::slope_mr(d0, d1, a1 - wl, th2, qs);
+        qmx0[v] = fma(-qs, mr, a0); qpx0[v] = fma(qs, mr, a0);
+        mr = pk::slope_mr(d1, d2, wr - a0, th2, qs);
+        qmx1[v] = fma(-qs, mr, a1);
+        qx[v * QXV + 1] = fma(qs, mr, a1);
+        mr = pk::slope_mr(a0 - wd.x, wu.x - a0, wu.x - wd.x, th2, qs);
+        qmy0[v] = fma(-qs, mr, a0);
+        const T qpy0 = fma(qs, mr, a0);
+        mr = pk::slope_mr(a1 - wd.y, wu.y - a1, wu.y - wd.y, th2, qs);
+        qmy1[v] = fma(-qs, mr, a1);
+        pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
+      }
+      if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
+      if (warp == ((c + 2) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
+      arrive(0);
     }
-    // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
+    // 2. z (between the two halves of the barrier): slope of cell c from this pair's own planes c-1 (dzm), c, c+1;
+    //    flux through the face between c-1 and c; finish cell c-1
     {
       T Gz[2][NV], qm[2][NV];
-#pragma unroll
-      for (int s = 0; s < 2; ++s)
+      {
+        const T *wn = wme + ((c + 1) & 1) * (NV * WV);
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
-          const T dp = Wn[s][v] - Wc[s][v];
-          T qs;
-          const T mr = pk::slope_mr(dzm[s][v], dp, dzm[s][v] + dp, th2, qs);
-          qm[s][v] = fma(-qs, mr, Wc[s][v]);
-          dzm[s][v] = dp;
-          Gz[s][v] = fma(qs, mr, Wc[s][v]);                        // q+ of cell c, parked until qpz has been used
+          const auto x = pk::ld2(wn + v * WV);
+          const T dp0 = x.x - Wc[0][v], dp1 = x.y - Wc[1][v];
+          T qs, mr;
+          mr = pk::slope_mr(dzm[0][v], dp0, dzm[0][v] + dp0, th2, qs);
+          qm[0][v] = fma(-qs, mr, Wc[0][v]);
+          Gz[0][v] = fma(qs, mr, Wc[0][v]);                        // q+ of cell c, parked until qpz has been used
+          mr = pk::slope_mr(dzm[1][v], dp1, dzm[1][v] + dp1, th2, qs);
+          qm[1][v] = fma(-qs, mr, Wc[1][v]);
+          Gz[1][v] = fma(qs, mr, Wc[1][v]);
+          dzm[0][v] = dp0; dzm[1][v] = dp1;
         }
+      }
       {
         T L0[NV], L1[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) { L0[v] = qpz[0][v]; L1[v] = qpz[1][v]; qpz[0][v] = Gz[0][v]; qpz[1][v] = Gz[1][v]; }
-        mk::floor_states2<T, NV>(L0, qm[0], L1, qm[1], P, hits);
         mk::face_flux<T, 2>(L0, qm[0], P, Gz[0]);
         mk::face_flux<T, 2>(L1, qm[1], P, Gz[1]);
       }
@@ -346,80 +406,61 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 #pragma unroll
       for (int v = 0; v < NV; ++v) { acc[0][v] = -Gz[0][v]; acc[1][v] = -Gz[1][v]; }   // the low z face enters with its sign
     }
-    if (live) {
-      // 3. x/y phase 1: slopes of both cells along x and y, publish the q+ the neighbours need
-      const T *w = wme + (c & 1) * (NV * WV);
-      T qmx0[NV], qpx0[NV], qmx1[NV], qmy0[NV], qmy1[NV];
+    if (!live) break;
+    mk::mbar_wait(&xbar[0], par);
+    // 3. fluxes through the low x and y faces of both cells
+    T Gx0[NV], Gx1[NV], Gy0[NV], Gy1[NV];
+    {
+      T WL[NV], WD0[NV], WD1[NV];
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
-        const T a0 = Wc[0][v], a1 = Wc[1][v];
-        const T wl = w[v * WV - 1], wr = w[v * WV + 2];
-        const auto wd = pk::ld2(w + v * WV - PW), wu = pk::ld2(w + v * WV + PW);
-        const T d0 = a0 - wl, d1 = a1 - a0, d2 = wr - a1;
-        T qs, mr;
-        mr = pk::slope_mr(d0, d1, a1 - wl, th2, qs);
-        qmx0[v] = fma(-qs, mr, a0); qpx0[v] = fma(qs, mr, a0);
-        mr = pk::slope_mr(d1, d2, wr - a0, th2, qs);
-        qmx1[v] = fma(-qs, mr, a1);
-        qx[v * QXV + 1] = fma(qs, mr, a1);
-        mr = pk::slope_mr(a0 - wd.x, wu.x - a0, wu.x - wd.x, th2, qs);
-        qmy0[v] = fma(-qs, mr, a0);
-        const T qpy0 = fma(qs, mr, a0);
-        mr = pk::slope_mr(a1 - wd.y, wu.y - a1, wu.y - wd.y, th2, qs);
-        qmy1[v] = fma(-qs, mr, a1);
-        pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
+        WL[v] = qx[v * QXV];
+        const auto y = pk::ld2(qy + v * QYV);
+        WD0[v] = y.x; WD1[v] = y.y;
       }
-      if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
-      if (warp == ((c + 2) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
-      __syncthreads();
-      if (tid == 0) {                              // ring slots that nobody reads any more
-        if (c + NSLOT - 1 < nz + 2 * NG) issue(c + NSLOT - 1);          // slot of plane c-1: cell c-1 is finished
-        if (BASE && c + 1 < NG + nz) issue_base(c + 1);                 // slot of cell c-1
+      mk::face_flux<T, 0>(WL, qmx0, P, Gx0);
+      mk::face_flux<T, 0>(qpx0, qmx1, P, Gx1);
+      mk::face_flux<T, 1>(WD0, qmy0, P, Gy0);
+      mk::face_flux<T, 1>(WD1, qmy1, P, Gy1);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { qx[v * QXV] = Gx0[v]; pk::st2(qy + v * QYV, Gy0[v], Gy1[v]); }
+    }
+    if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo);
+    if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo);
+    arrive(1);
+    if (bflux) {
+      if ((i0 & 7) == 0) {
+        T *B = bflux + ((size_t(pl) * 9 + 0 + (i0 >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + j;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx0[v];
       }
-      // 4. phase 2: fluxes through the low x and y faces of both cells
-      T Gx0[NV], Gx1[NV], Gy0[NV], Gy1[NV];
-      {
-        T WL[NV], WD0[NV], WD1[NV];
+      if ((j & 7) == 0) {
+        T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + i0;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) {
-          WL[v] = qx[v * QXV];
-          const auto y = pk::ld2(qy + v * QYV);
-          WD0[v] = y.x; WD1[v] = y.y;
-        }
-        pk::floor_faces4<T, NV>(WL, qmx0, qpx0, qmx1, WD0, qmy0, WD1, qmy1, P, hits);
-        mk::face_flux<T, 0>(WL, qmx0, P, Gx0);
-        mk::face_flux<T, 0>(qpx0, qmx1, P, Gx1);
-        mk::face_flux<T, 1>(WD0, qmy0, P, Gy0);
-        mk::face_flux<T, 1>(WD1, qmy1, P, Gy1);
-#pragma unroll
-        for (int v = 0; v < NV; ++v) { qx[v * QXV] = Gx0[v]; pk::st2(qy + v * QYV, Gy0[v], Gy1[v]); }
-      }
-      if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo, hits);
-      if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo, hits);
-      if (bflux) {
-        if ((i0 & 7) == 0) {
-          T *B = bflux + ((size_t(pl) * 9 + 0 + (i0 >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + j;
-#pragma unroll
-          for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx0[v];
-        }
-        if ((j & 7) == 0) {
-          T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + i0;
-#pragma unroll
-          for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gy0[v], T(0.5) * Gy1[v]);
-        }
-      }
-      __syncthreads();
-      // 5. phase 3: flux differences in x and y (the low z face is already in acc)
-#pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const T fxh = qx[v * QXV + 1];
-        const auto fyh = pk::ld2(qy + v * QYV + NI);
-        acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) + acc[0][v];
-        acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) + acc[1][v];
+        for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gy0[v], T(0.5) * Gy1[v]);
       }
     }
+    // 4. (between the two halves of the second barrier) plane c+2: raw -> primitives, published for iteration c+2;
+    //    every thread has passed the first barrier, so nobody reads plane c in that buffer any more
+    if (c + 2 < nz + 2 * NG) {
+      T Wa[NV], Wb[NV];
+      const bool hl = c + 2 < NG + nz;
+      convert(c + 2, hl, Wa, Wb);
+      if (c + 3 < NG + nz) halo_load(c + 3);
+    }
+    mk::mbar_wait(&xbar[1], par);
+    if (tid == 0) {                                // every thread is past step 2: these ring slots are free
+      if (c + NSLOT - 1 < nz + 2 * NG) issue(c + NSLOT - 1);            // slot of plane c-1
+      if (BASE && c + 1 < NG + nz) issue_base(c + 1);                   // slot of cell c-1
+    }
+    // 5. flux differences in x and y (the low z face is already in acc)
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { Wc[0][v] = Wn[0][v]; Wc[1][v] = Wn[1][v]; }
+    for (int v = 0; v < NV; ++v) {
+      const T fxh = qx[v * QXV + 1];
+      const auto fyh = pk::ld2(qy + v * QYV + NI);
+      acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) + acc[0][v];
+      acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) + acc[1][v];
+    }
   }
   if (BASE && smax_out) {
     // one atomicMax per warp on the bit pattern of a non-negative double (monotone as an unsigned integer)
