@@ -47,6 +47,7 @@ def parse():
     ap.add_argument("--halo", type=int, default=1, help="1: rk_stage reads sibling interiors directly")
     ap.add_argument("--kernel", type=int, default=2)
     ap.add_argument("--zsplit", type=int, default=2, help="AMRHYDRO_OPT_ZSPLIT (2 = automatic)")
+    ap.add_argument("--fuse-cfl", type=int, default=2, help="AMRHYDRO_OPT_FUSE_CFL (2 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -228,7 +229,7 @@ def run_ours(args):
     single = h["nlevels"] == 1
     esz = 8 if args.dtype == "f64" else 4
     npdt = np.float64 if args.dtype == "f64" else np.float32
-    g = binding.AmrHydro(h, gamma, nv, dtype=args.dtype, halo=args.halo, kernel=args.kernel, zsplit=args.zsplit, device="cuda:%d" % local)
+    g = binding.AmrHydro(h, gamma, nv, dtype=args.dtype, halo=args.halo, kernel=args.kernel, zsplit=args.zsplit, fuse_cfl=args.fuse_cfl, device="cuda:%d" % local)
     host_in = torch.empty((npatch, nv, 16, 16, 16), dtype=torch.float64 if esz == 8 else torch.float32, pin_memory=True)
     host_in.numpy()[...] = U.astype(npdt, copy=False)
     del U

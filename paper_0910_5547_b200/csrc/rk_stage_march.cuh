@@ -57,10 +57,9 @@ __device__ __forceinline__ float frcp(float x) {
 __device__ __forceinline__ double fsqrt(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double g = x * y, h = 0.5 * y;
-  double r = fma(-g, h, 0.5);              // (1 - x y^2)/2
-  r = r * fma(1.5, r, 1.0);                // (1-2r)^(-1/2) = 1 + r + 1.5 r^2 + O(r^3)
-  return fma(g, r, g);
+  const double g = x * y;
+  const double r = fma(-g, y, 1.0);              // 1 - x y^2
+  return fma(g * r, fma(0.375, r, 0.5), g);      // g (1-r)^(-1/2) = g (1 + r/2 + 3/8 r^2 + O(r^3)): five FP64 operations
 }
 __device__ __forceinline__ float fsqrt(float x) {
   float y;

@@ -404,7 +404,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         }
       }
 #pragma unroll
-      for (int v = 0; v < NV; ++v) { acc[0][v] = -Gz[0][v]; acc[1][v] = -Gz[1][v]; }   // the low z face enters with its sign
+      for (int v = 0; v < NV; ++v) { acc[0][v] = Gz[0][v]; acc[1][v] = Gz[1][v]; }     // the low z face (subtracted in step 5)
     }
     if (!live) break;
     mk::mbar_wait(&xbar[0], par);
@@ -453,13 +453,13 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       if (c + NSLOT - 1 < nz + 2 * NG) issue(c + NSLOT - 1);            // slot of plane c-1
       if (BASE && c + 1 < NG + nz) issue_base(c + 1);                   // slot of cell c-1
     }
-    // 5. flux differences in x and y (the low z face is already in acc)
+    // 5. flux differences in x and y, minus the low z face parked in acc
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const T fxh = qx[v * QXV + 1];
       const auto fyh = pk::ld2(qy + v * QYV + NI);
-      acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) + acc[0][v];
-      acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) + acc[1][v];
+      acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) - acc[0][v];
+      acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) - acc[1][v];
     }
   }
   if (BASE && smax_out) {
@@ -478,7 +478,10 @@ int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sba
                          T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0) {
   static bool configured = false;
-  constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES, bytes1 = pk::Smem<T, NV, true>::BYTES;
+#ifndef AMR_PAIR_EXTRA_SMEM
+#define AMR_PAIR_EXTRA_SMEM 0     // experiment: pad the allocation to force one CTA per SM
+#endif
+  constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES + AMR_PAIR_EXTRA_SMEM, bytes1 = pk::Smem<T, NV, true>::BYTES + AMR_PAIR_EXTRA_SMEM;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_rk_stage_pair<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
     if (e == cudaSuccess)
