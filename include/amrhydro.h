@@ -48,22 +48,18 @@ extern "C" {
 #define AMRHYDRO_OPT_THETA 2      /* limiter parameter of Eq. 9-10, 0..2 (default 1.5, S1); any time */
 #define AMRHYDRO_OPT_RHO_FLOOR 3  /* S11, default 1e-30; any time                                  */
 #define AMRHYDRO_OPT_EINT_FLOOR 4 /* S11, default 1e-30; any time                                  */
-#define AMRHYDRO_OPT_KERNEL 5     /* rk_stage variant: 0 = reference one-thread-per-cell kernel,
-                                     1 = z-marching shared-memory kernel (first version),
-                                     2 = TMA-fed z-marching kernel (default),
-                                     3 = its register-light variant (two CTAs per SM),
-                                     4 = the same on quarter-patch 8x8 tiles (3-warp CTAs);
-                                     3 and 4 are measured alternatives (profiles/README.md),
-                                     all five agree to round-off; any time                         */
-#define AMRHYDRO_OPT_HALO 6       /* 0 = rk_stage reads materialised ghost zones (default);
-                                     1 = rk_stage reads sibling interiors directly, fill_ghosts
-                                     then only writes coarse-fine / physical faces; any time      */
-#define AMRHYDRO_OPT_FUSE_CFL 7   /* the combination stage (a != 0) of the default rk_stage kernel can also reduce
-                                     the max signal speed of the state it writes, so that the next
-                                     amrhydro_cfl_dt of that slot launches nothing: 0 = never, 1 = always,
-                                     2 (default) = in fp32 only, where it costs nothing (measured at 512^3:
-                                     fp32 step 6.89 -> 6.09 ms; fp64 step 14.72 -> 14.26 ms but the FP64-pipe
-                                     bound stage grows by 0.57 ms); any time                          */
+#define AMRHYDRO_OPT_KERNEL 5     /* rk_stage variant: 0 = reference one-thread-per-cell kernel (cross-check),
+                                     2 = k_rk_stage_march (one cell per thread, 8 + 2 halo warps per patch),
+                                     3 (default) = k_rk_stage_pair for nvars = 5 (two cells per thread, 4 warps per
+                                     patch, two CTAs per SM; measured faster, profiles/README.md) and
+                                     k_rk_stage_march for nvars = 8, 9; all agree to round-off; any time        */
+#define AMRHYDRO_OPT_HALO 6       /* 1 (default) = rk_stage reads sibling interiors directly, fill_ghosts then only
+                                     writes coarse-fine / physical faces (and sibling ghosts on levels someone
+                                     prolongates from); 0 = rk_stage reads materialised ghost zones; any time   */
+#define AMRHYDRO_OPT_FUSE_CFL 7   /* the combination stage (a != 0) of rk_stage can also reduce the max signal speed of
+                                     the state it writes, so that the next amrhydro_cfl_dt of that slot launches
+                                     nothing: 0 = never, 1 or 2 (default) = always (measured at 512^3: fp32 step
+                                     6.89 -> 6.09 ms, fp64 11.65 -> 10.88 ms); any time                          */
 
 #define AMRHYDRO_OPT_GLM_CH 8     /* nvars = 9: c_h of Eq. 15 (S17), > 0, default 1; any time               */
 #define AMRHYDRO_OPT_GLM_CR 9     /* nvars = 9: c_r = c_p^2/c_h of the psi damping applied by amrhydro_advance

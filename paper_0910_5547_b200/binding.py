@@ -82,7 +82,7 @@ class AmrHydroError(RuntimeError):
 class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
-    def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=2, halo=0,
+    def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=3, halo=1,
                  rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():

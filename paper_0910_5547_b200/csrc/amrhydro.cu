@@ -28,7 +28,7 @@ struct amrhydro {
   int nv = 5, bits = 64;
   double theta = 1.5, rho_floor = 1e-30, e_floor = 1e-30;
   double glm_ch = 1.0, glm_cr = 0.18;      // S17, S18 (nvars = 9)
-  int kernel = 2, halo = 0;
+  int kernel = 3, halo = 1;                 // rk_stage_pair for nvars = 5 (rk_stage_march otherwise); direct sibling halos
   void *pool = nullptr;
   size_t pool_bytes = 0;
   int maxp = 0, nslots = 0;
@@ -49,7 +49,7 @@ struct amrhydro {
   std::vector<int> smax_slot;               // slot the cached value belongs to, -1 = stale
   int zsplit = 2;                           // rk_stage_march: 0 never, 1 always, 2 = levels of at most num_sms/2 patches
   int num_sms = 148;
-  int fuse_cfl = 2;                         // 0 never, 1 always, 2 = where it is free (fp32)
+  int fuse_cfl = 2;                         // 0 never, 1 / 2 = the combination stage also reduces the max signal speed
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
@@ -149,6 +149,8 @@ void free_hierarchy(amrhydro *h) {
 
 extern "C" {
 
+static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot);
+
 amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) {
   if (!(gamma > 1.0) || (nvars != 5 && nvars != 8 && nvars != 9) || patch_dim != NI || nghost != NG) return nullptr;
   int ndev = 0;
@@ -163,6 +165,7 @@ amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) 
   }
   if (cudaMalloc(&h->d_scalars, 2 * sizeof(unsigned long long)) != cudaSuccess) { delete h; return nullptr; }
   cudaMemset(h->d_scalars, 0, 2 * sizeof(unsigned long long));
+  cudaDeviceSynchronize();                 // (legacy-stream memset; later work runs on the caller's stream)
   return h;
 }
 
@@ -282,6 +285,10 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
     for (int r = 0; r < 27; ++r)
       if (r != 13 && (d.nbr[r] >= np || d.nbr[r] < -2 || (d.nbr[r] >= 0 && tbl[d.nbr[r]].level != d.level)))
         return fail(h, AMRHYDRO_EINVAL, "bad neighbour entry");
+    for (int f = 0; f < 6; ++f)                // no kernel fills a physical ghost zone on a periodic side
+      if (d.nbr[face_region(f)] == AMRHYDRO_NBR_PHYSICAL && bc[f] == AMRHYDRO_BC_PERIODIC)
+        return fail(h, AMRHYDRO_EINVAL, "physical-boundary neighbour entry on a periodic side");
+    if (d.level == 0 && d.parent != -1) return fail(h, AMRHYDRO_EINVAL, "level-0 patches have parent -1");
     if (d.level == 0) {
       for (int r = 0; r < 27; ++r)
         if (r != 13 && d.nbr[r] == -1) return fail(h, AMRHYDRO_EINVAL, "level 0 cannot have coarse-fine faces");
@@ -307,6 +314,24 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
   }
   for (int l = 0; l < nlev; ++l)
     if (count[l] == 0) return fail(h, AMRHYDRO_EINVAL, "empty level");
+  {
+    // the domain extent follows from level 0: a face is AMRHYDRO_NBR_PHYSICAL if and only if the patch touches that
+    // side of the domain (on non-periodic sides)
+    int lo0[3] = {1 << 30, 1 << 30, 1 << 30}, hi0[3] = {-(1 << 30), -(1 << 30), -(1 << 30)};
+    for (int p = 0; p < np && tbl[p].level == 0; ++p)
+      for (int a = 0; a < 3; ++a) {
+        lo0[a] = std::min(lo0[a], tbl[p].origin[a]);
+        hi0[a] = std::max(hi0[a], tbl[p].origin[a] + NI);
+      }
+    for (int p = 0; p < np; ++p)
+      for (int f = 0; f < 6; ++f) {
+        const int a = f >> 1, l = tbl[p].level;
+        const bool touches = (f & 1) ? (tbl[p].origin[a] + NI == (hi0[a] << l)) : (tbl[p].origin[a] == (lo0[a] << l));
+        const bool phys = tbl[p].nbr[face_region(f)] == AMRHYDRO_NBR_PHYSICAL;
+        if (bc[f] != AMRHYDRO_BC_PERIODIC && phys != touches)
+          return fail(h, AMRHYDRO_EINVAL, "physical-boundary face entries must match the faces on the domain boundary");
+      }
+  }
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   free_hierarchy(h);
   h->tbl.assign(tbl, tbl + np);
@@ -326,20 +351,22 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
   CUDA_TRY(h, cudaMalloc(&h->d_desc, size_t(np) * sizeof(Desc)));
   CUDA_TRY(h, cudaMalloc(&h->d_child, size_t(np) * 8 * sizeof(int)));
   CUDA_TRY(h, cudaMalloc(&h->d_octant, size_t(np) * sizeof(int)));
-  CUDA_TRY(h, cudaMemcpy(h->d_desc, tbl, size_t(np) * sizeof(Desc), cudaMemcpyHostToDevice));
-  CUDA_TRY(h, cudaMemcpy(h->d_child, child.data(), size_t(np) * 8 * sizeof(int), cudaMemcpyHostToDevice));
-  CUDA_TRY(h, cudaMemcpy(h->d_octant, octant.data(), size_t(np) * sizeof(int), cudaMemcpyHostToDevice));
+  // (h->tbl / h->child / h->octant are the handle's own copies: they outlive the asynchronous uploads)
+  CUDA_TRY(h, cudaMemcpyAsync(h->d_desc, h->tbl.data(), size_t(np) * sizeof(Desc), cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(h, cudaMemcpyAsync(h->d_child, h->child.data(), size_t(np) * 8 * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(h, cudaMemcpyAsync(h->d_octant, h->octant.data(), size_t(np) * sizeof(int), cudaMemcpyHostToDevice, h->stream));
   if (nlev > 1) {
     size_t rb = size_t(np) * 6 * h->nv * 64 * elem(h);
     CUDA_TRY(h, cudaMalloc(&h->d_Rf, rb));
     CUDA_TRY(h, cudaMalloc(&h->d_Rc, rb));
-    CUDA_TRY(h, cudaMemset(h->d_Rf, 0, rb));
-    CUDA_TRY(h, cudaMemset(h->d_Rc, 0, rb));
+    CUDA_TRY(h, cudaMemsetAsync(h->d_Rf, 0, rb, h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(h->d_Rc, 0, rb, h->stream));
     size_t mx = *std::max_element(count.begin(), count.end());
     CUDA_TRY(h, cudaMalloc(&h->d_bflux, mx * 9 * h->nv * 256 * elem(h)));
     h->bflux_patches = mx;
   }
   h->np = np;
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));   // the pageable-memory copies above are staged: make them final
   return 0;
 }
 
@@ -397,6 +424,7 @@ int amrhydro_download_padded(amrhydro_t *h, int slot, int patch, double *out) {
   if (!out || patch < 0 || patch >= h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch");
   size_t bytes = size_t(h->nv) * NP * NP * NP * sizeof(double);
   if (int r = ensure_stage(h, bytes)) return r;
+  if (int r = materialise_sibling_ghosts(h, h->tbl[patch].level, slot)) return r;
   int r = dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     k_unpack_padded<T><<<64, 256, 0, h->stream>>>(make_pool<T>(h), slot, patch, (double *)h->d_stage);
@@ -486,7 +514,7 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
     pold = pnew = slot;
   }
   // direct-halo mode: sibling copies are only needed where someone prolongates from this level
-  const int skip = (h->halo == 1 && level + 1 >= h->nlev) ? 1 : 0;
+  const int skip = (h->halo == 1 && level + 1 >= h->nlev) ? 1 : 0;   // (mode bit 0 of k_fill_ghosts)
   const bool phase1 = !skip || h->lev_has_cf[level], phase2 = h->lev_has_phys[level];
   if (!phase1 && !phase2) return 0;   // e.g. periodic single level with direct halos: nothing to materialise
   return dispatch(h, [&](auto t, auto nv) {
@@ -506,6 +534,20 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
   });
 }
 
+// Calls that read a patch's own padded box (refine_indicator, download_padded) need the sibling ghosts that
+// fill_ghosts leaves out in direct-halo mode on the finest level: copy them now (siblings only, no prolongation).
+static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot) {
+  if (!(h->halo == 1 && level + 1 >= h->nlev)) return 0;
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    constexpr int NV = decltype(nv)::value;
+    k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
+        make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2);
+    LAUNCH_CHECK(h);
+    return 0;
+  });
+}
+
 int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, double a, double b, double dt, double w) {
   if (int r = check_ready(h)) return r;
   if (int r = check_level(h, level)) return r;
@@ -520,7 +562,7 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
     smax_touch(h, level, sout);
     // the combination stage can also reduce the max signal speed of what it writes (a1 fused into a6)
-    const bool fuse = h->kernel != 0 && (h->fuse_cfl == 1 || (h->fuse_cfl == 2 && h->bits == 32)) && a != 0.0;
+    const bool fuse = h->kernel != 0 && h->fuse_cfl != 0 && a != 0.0;
     const int zs = (h->zsplit == 1 || (h->zsplit == 2 && 2 * n <= h->num_sms)) ? 1 : 0;
     if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
     if (h->kernel == 0) {
@@ -611,6 +653,7 @@ int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_o
   const size_t bytes = size_t(n) * 8 * sizeof(double);
   if (int r = ensure_stage(h, bytes)) return r;
   const double inv2dx = 0.5 / (h->dx0 / double(1 << level));
+  if (int r = materialise_sibling_ghosts(h, level, slot)) return r;
   int r = dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     k_refine_indicator<T><<<n, 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level], inv2dx, (double *)h->d_stage);

@@ -70,7 +70,10 @@ __global__ void __launch_bounds__(256) k_cfl(Pool<T> pool, int slot, int first, 
     for (int v = 0; v < NV; ++v) U[v] = Ub[size_t(v) * Layout<T>::VS + c];
     cons_to_prim<T, NV>(U, W, P, hits);
     T s = max_signal_speed<T, NV>(W, P);
-    const T chk = ((W[2] + W[3]) + W[4]) + s;      // fmax drops NaNs: test the operands themselves
+    // fmax drops NaNs and the floors replace a NaN density or energy: test the raw conserved inputs and the result
+    T chk = s;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) chk += U[v];
     bad |= !(chk - chk == T(0));                   // NaN or inf anywhere
     best = tmax(best, s);
   }
@@ -101,13 +104,14 @@ template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
 // copied from that sibling's interior; where it is a coarse-fine boundary it is prolongated
 // from the parent's padded box, conservative limited-linear (S6) in time-interpolated parent
 // data (S7; alpha = 0 or 1 reads only the slot that counts, which is the same value bitwise for
-// finite data).  skip_siblings: face/edge/corner copies are skipped (rk_stage reads siblings directly).
+// finite data).  mode bit 0: sibling face/edge/corner copies are skipped (rk_stage reads siblings directly);
+// bit 1: the prolongation is skipped (siblings only: refine_indicator / download_padded in direct-halo mode).
 // Phase 2 (k_fill_outflow, launched only for levels that touch an outflow boundary): zero-gradient
 // outflow, x then y then z over the full padded extent, one block per patch.
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
                                                      int first, const Desc *__restrict__ desc,
-                                                     const int *__restrict__ octant, int skip_siblings) {
+                                                     const int *__restrict__ octant, int mode) {
   // Latency is what this kernel costs on small AMR levels, so it is written as two dependent round trips to
   // memory: (1) the patch's descriptor row and octant (every thread reads what it needs, broadcast through
   // L1: no staging, no barrier), (2) all parent cells this plane prolongates from -- 3 coarse planes x 12 x 12
@@ -123,7 +127,8 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
   const int *nbr = D.nbr + (oz + 1) * 9;             // the nine regions of this plane
   bool cf = false;                                   // block-uniform: does this plane touch a coarse-fine region?
-  if (Q >= 0) {
+  const bool skip_siblings = mode & 1;
+  if (Q >= 0 && !(mode & 2)) {
 #pragma unroll
     for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
   }

@@ -537,7 +537,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
           T Wq[NV];
           mk::prim<T, NV>(un, Wq, P, hits);
           const T sp = mk::max_speed_fast<T, NV>(Wq, P);
-          const T chk = ((Wq[2] + Wq[3]) + Wq[4]) + sp;
+          const T chk = (((Wq[2] + Wq[3]) + Wq[4]) + sp) + (un[0] + un[4]);   // (the floors would hide a NaN density or energy)
           bad |= !(chk - chk == T(0));
           best = tmax(best, sp);
         }

@@ -62,6 +62,29 @@ def test_errors_are_reported_and_do_not_poison_the_handle(gpu):
     assert g.L.amrhydro_create(1.4, 5, 32, 2) is None and g.L.amrhydro_create(1.4, 5, 16, 3) is None
 
 
+def test_set_hierarchy_rejects_tables_no_kernel_can_fill(gpu):
+    """A physical-boundary entry on a periodic side (nothing would fill that ghost zone), a physical entry on an
+    interior face, an interior entry on a boundary face, and a level-0 patch with a parent."""
+    import copy
+    h = wl.uniform_hierarchy(2, periodic=True)
+    bad = copy.deepcopy(h); bad["nbr"] = h["nbr"].copy(); bad["nbr"][0, 12] = -2
+    with pytest.raises(gpu.AmrHydroError):
+        gpu.AmrHydro(bad, 1.4, 5)
+    h = wl.uniform_hierarchy(2, periodic=False)
+    gpu.AmrHydro(h, 1.4, 5)                                         # the generator's own table is accepted
+    bad = copy.deepcopy(h); bad["nbr"] = h["nbr"].copy()
+    p = int(np.argmax((h["origin"] == 0).all(axis=1)))              # the corner patch: its x-hi face is interior
+    bad["nbr"][p, 14] = -2
+    with pytest.raises(gpu.AmrHydroError):
+        gpu.AmrHydro(bad, 1.4, 5)
+    bad = copy.deepcopy(h); bad["nbr"] = h["nbr"].copy(); bad["nbr"][p, 12] = int(h["nbr"][p, 14])   # x-lo is on the boundary
+    with pytest.raises(gpu.AmrHydroError):
+        gpu.AmrHydro(bad, 1.4, 5)
+    bad = copy.deepcopy(h); bad["parent"] = h["parent"].copy(); bad["parent"][0] = 1
+    with pytest.raises(gpu.AmrHydroError):
+        gpu.AmrHydro(bad, 1.4, 5)
+
+
 @pytest.mark.parametrize("nb,periodic", [((3, 1, 2), True), ((1, 1, 1), False), ((1, 4, 1), False)])
 @pytest.mark.parametrize("halo", [0, 1])
 def test_non_cubic_and_one_patch_thick_grids(gpu, nb, periodic, halo):

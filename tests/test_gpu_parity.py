@@ -111,12 +111,31 @@ def test_cfl_dt_reports_nonfinite(gpu):
         g.cfl_dt(0, 0, 0.3)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("fuse", [0, 1])
+@pytest.mark.parametrize("var,val", [(0, np.nan), (4, np.nan), (0, -np.nan), (4, np.inf), (2, np.nan)])
+def test_nonfinite_density_or_energy_is_not_masked_by_the_floors(gpu, dtype, fuse, var, val):
+    """The floors of S11 replace a NaN density or energy: the reduction must still report it, with the
+    stand-alone kernel (fuse = 0) and with the reduction fused into the combination stage alike."""
+    h = wl.uniform_hierarchy(2, periodic=True)
+    U = rand_state(h, 5, 23)
+    U[5, var, 7, 8, 9] = val
+    g = gpu.AmrHydro(h, 1.4, 5, dtype=dtype, fuse_cfl=fuse)
+    g.upload(0, U)
+    with pytest.raises(gpu.AmrHydroError):          # stand-alone reduction of the uploaded state
+        g.cfl_dt(0, 0, 0.3)
+    g.fill_ghosts(0, 0)
+    g.rk_stage(0, 0, 0, 1, 0.5, 0.5, 1e-3)          # combination stage: writes slot 1 (and its maximum when fused)
+    with pytest.raises(gpu.AmrHydroError):
+        g.cfl_dt(0, 1, 0.3)
+
+
 # ------------------------------------------------------------------ a2: ghost fill
 @pytest.mark.parametrize("periodic", [True, False])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_fill_ghosts_single_level_bit_exact(gpu, periodic, dtype):
     h = wl.uniform_hierarchy(2, periodic=periodic)
-    g, o = make_pair(gpu, h, 1.4, 5, dtype)
+    g, o = make_pair(gpu, h, 1.4, 5, dtype, halo=0)          # materialised ghosts: the whole padded box is defined
     upload_both(g, o, rand_state(h, 5, 3), dtype)
     g.fill_ghosts(0, 0); o.fill_ghosts(0, 0)
     P = o.download_padded(0)

@@ -38,13 +38,16 @@ def blob_state(h, nv=5, amp=5.0, w=0.12, seed=0, noise=0.01):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("periodic", [True, False])
-def test_refine_indicator_matches_oracle(gpu, dtype, periodic):
+@pytest.mark.parametrize("halo", [0, 1])
+def test_refine_indicator_matches_oracle(gpu, dtype, periodic, halo):
+    """halo = 1: fill_ghosts leaves the sibling ghosts of the finest level to rk_stage's direct reads; the
+    indicator materialises them itself before it differentiates across patch borders."""
     import oracle
     h = wl.uniform_hierarchy(3, periodic=periodic)
     U = blob_state(h)
     if dtype == "f32":
         U = U.astype(np.float32).astype(np.float64)
-    g = gpu.AmrHydro(h, 1.4, 5, dtype=dtype)
+    g = gpu.AmrHydro(h, 1.4, 5, dtype=dtype, halo=halo)
     o = oracle.Oracle(h, 1.4, 5)
     g.upload(0, U); o.upload(0, U)
     g.fill_ghosts(0, 0); o.fill_ghosts(0, 0)
@@ -55,6 +58,25 @@ def test_refine_indicator_matches_oracle(gpu, dtype, periodic):
     U[5, 0, 3, 4, 5] = np.nan
     g.upload(0, U); g.fill_ghosts(0, 0)
     assert np.isnan(g.refine_indicator(0)[5]).any()
+
+
+@pytest.mark.parametrize("halo", [0, 1])
+def test_refine_indicator_on_the_finest_level_of_a_hierarchy(gpu, halo):
+    """The same on the fine level of a two-level hierarchy (coarse-fine faces prolongated by fill_ghosts,
+    sibling faces materialised by the indicator in direct-halo mode) and on its coarse level."""
+    import oracle
+    fine = [(i, j, k) for i in (2, 3) for j in (2, 3) for k in (2, 3)]
+    h = wl.build_hierarchy((3, 3, 3), [fine], (0,) * 6)
+    U = blob_state(h, w=0.2)
+    g = gpu.AmrHydro(h, 1.4, 5, halo=halo)
+    o = oracle.Oracle(h, 1.4, 5)
+    g.upload(0, U); o.upload(0, U)
+    for lev in (0, 1):
+        g.fill_ghosts(lev, 0, 0, 0, 0.0); o.fill_ghosts(lev, 0, 0, 0, 0.0)
+    for lev in (0, 1):
+        G, O = g.refine_indicator(lev), o.refine_indicator(lev)
+        assert G.shape == O.shape and O.max() > 0.5
+        assert np.abs(G - O).max() <= 1e-13 * O.max()
 
 
 @pytest.mark.parametrize("nv,dtype", [(5, "f64"), (8, "f64"), (5, "f32")])
