@@ -108,6 +108,28 @@ def prim(nvars, gamma, U):
     return W
 
 
+def face_floors(nvars, gamma, theta, direction, rho_floor, e_floor, Wm2, Wm1, W0, Wp1):
+    """face() with the floors of S11 given explicitly.  Returns (WL, WR, lambda0, F, floor activations)."""
+    arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (Wm2, Wm1, W0, Wp1)]
+    WL, WR, F = (np.zeros(nvars) for _ in range(3))
+    hits = C.c_long(0)
+    f = lib().orc_face_floors
+    f.restype = C.c_double
+    lam = f(C.c_int(nvars), C.c_double(gamma), C.c_double(theta), C.c_int(direction), C.c_double(rho_floor),
+            C.c_double(e_floor), *[_dp(a) for a in arrs], _dp(WL), _dp(WR), _dp(F), C.byref(hits))
+    return WL, WR, lam, F, hits.value
+
+
+def prim_floors(nvars, gamma, rho_floor, e_floor, U):
+    """prim() with the floors of S11 given explicitly.  Returns (W, floor activations)."""
+    U = np.ascontiguousarray(U, dtype=np.float64)
+    W = np.zeros(nvars)
+    hits = C.c_long(0)
+    lib().orc_prim_floors(C.c_int(nvars), C.c_double(gamma), C.c_double(rho_floor), C.c_double(e_floor), _dp(U), _dp(W),
+                          C.byref(hits))
+    return W, hits.value
+
+
 def flux(nvars, gamma, direction, W):
     """(U(W), F^d(W), signal speed along d) of one primitive state."""
     W = np.ascontiguousarray(W, dtype=np.float64)

@@ -742,6 +742,19 @@ double orc_face(int nvars, double gamma, double theta, int dir, const double *Wm
   q.plm(Wm2, Wm1, W0, Wp1, WL, WR);
   return q.riemann(WL, WR, dir, F);
 }
+// the same two helpers with the floors of S11 given by the caller and their activations counted (pin P20:
+// tests/test_oracle_pins.py drives states below the floors through them); no arithmetic of their own
+double orc_face_floors(int nvars, double gamma, double theta, int dir, double rho_floor, double e_floor, const double *Wm2,
+                       const double *Wm1, const double *W0, const double *Wp1, double *WL, double *WR, double *F,
+                       long *hits) {
+  Phys<double> q{nvars, gamma, theta, rho_floor, e_floor, hits};
+  q.plm(Wm2, Wm1, W0, Wp1, WL, WR);
+  return q.riemann(WL, WR, dir, F);
+}
+void orc_prim_floors(int nvars, double gamma, double rho_floor, double e_floor, const double *U, double *W, long *hits) {
+  Phys<double> q{nvars, gamma, 1.5, rho_floor, e_floor, hits};
+  q.prim(U, W);
+}
 void orc_prim(int nvars, double gamma, const double *U, double *W) {
   Phys<double> q{nvars, gamma, 1.5, 1e-300, 1e-300, nullptr};
   q.prim(U, W);

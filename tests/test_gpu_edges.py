@@ -131,7 +131,7 @@ def test_sedov_amr_fp32_and_direct_halos(gpu, dtype, halo):
         g.advance(0.3, dt)
     G, O = g.download(0).astype(np.float64), o.download(0)
     assert np.isfinite(G).all()
-    assert norm_err(G, O, vector=(dtype == "f32")).max() <= (1e-12 if dtype == "f64" else 1e-5)
+    assert norm_err(G, O, vector=(dtype == "f32"), label="Sedov AMR 32^3+2 halo=%d" % halo).max() <= (1e-12 if dtype == "f64" else 1e-5)
 
 
 @pytest.mark.parametrize("dtype,nv", [("f64", 5), ("f32", 5), ("f64", 8), ("f64", 9)])

@@ -1,11 +1,14 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
-(direct sibling halos, default stage kernel), on sampled patches the oracle can compute one by one.
+(library defaults: direct sibling halos, default stage kernel, fused CFL reduction), on sampled patches
+the oracle can compute one by one, over the run lengths of SURVEY.md 8(d): 10 steps (configs 2 and 4),
+3 steps (config 5).
 
-One RK2 step of a patch depends on data within 4 cells of it (2 per stage), so the oracle run on
-the 3x3x3 block of patches around a sampled patch (48^3 cells, made periodic: its outer wrap is
-more than 4 cells away from the centre patch) reproduces that patch of the full-size run exactly.
-The time step is the GPU's own cfl_dt of the full level, checked against the oracle's max wave
-speed on the sampled blocks (which can only be smaller or equal).
+One RK2 step of a patch depends on data within 4 cells of it (2 per stage), k steps on 4k cells.  The oracle
+run on the (2r+1)^3 block of patches around a sampled patch, r = ceil(4k/16), made periodic, reproduces that
+patch of the full-size run exactly: the block's wrap-around is more than 4k cells from the centre patch
+(r = 1: the 3^3 block up to 4 steps; r = 3: 7^3 patches for 10 steps).  Every step uses the GPU's own time
+step of the full level (its fused / stand-alone CFL reduction), handed to the oracle, and checked against the
+oracle's max wave speed on the sampled blocks (which can only be smaller or equal).
 """
 import numpy as np
 import pytest
@@ -26,67 +29,62 @@ def gpu():
     return binding
 
 
-def block_around(G, bx, by, bz, nb):
-    """48^3 cells (3x3x3 patches) of the periodic global array G[nv][z][y][x] centred on patch (bx,by,bz)."""
-    idx = lambda b: np.arange((b - 1) * 16, (b + 2) * 16) % (nb * 16)
+def block_around(G, bx, by, bz, nb, r):
+    """(2r+1)^3 patches of the periodic global array G[nv][z][y][x] centred on patch (bx,by,bz)."""
+    idx = lambda b: np.arange((b - r) * 16, (b + r + 1) * 16) % (nb * 16)
     return G[:, idx(bz)][:, :, idx(by)][:, :, :, idx(bx)]
 
 
-def check_fullsize(gpu, G, gamma, nv, dtype, nsample, seed, tol, cfl=0.3):
+def check_fullsize(gpu, G, gamma, nv, dtype, nsample, seed, tol, steps, label, cfl=0.3):
     import oracle
     n = G.shape[-1]
     nb = n // 16
+    r = -(-4 * steps // 16)
+    assert 2 * r + 1 <= nb
     h = wl.uniform_hierarchy(nb, periodic=True)
     U = wl.split_global(h, G)
     if dtype == "f32":
         U = U.astype(np.float32)
         G = G.astype(np.float32).astype(np.float64)      # S15: the oracle starts from the rounded data
-    g = gpu.AmrHydro(h, gamma, nv, dtype=dtype, halo=1)
+    g = gpu.AmrHydro(h, gamma, nv, dtype=dtype)          # library defaults = what bench.py times
     g.upload(0, U)
     del U
-    dt = g.cfl_dt(0, 0, cfl)
-    g.fill_ghosts(0, 0)
-    g.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
-    g.fill_ghosts(0, 1)
-    g.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+    dts = [g.advance(cfl) for _ in range(steps)]         # the GPU's own dt of the full level, every step
     assert g.get_counter(gpu.CNT_FLOOR_HITS) == 0
     org = np.asarray(h["origin"]) // 16
     rng = np.random.default_rng(seed)
-    picks = list(rng.choice(len(org), size=nsample - 2, replace=False)) + [0, len(org) - 1]   # incl. wrap-around patches
-    hb = wl.build_hierarchy((3, 3, 3), (), (0,) * 6, box=48.0 / n, order="linear")   # periodic, same cell size as the full level
+    picks = list(rng.choice(len(org), size=max(0, nsample - 2), replace=False)) + [0, len(org) - 1]   # incl. wrap-around patches
+    m = 2 * r + 1
+    hb = wl.build_hierarchy((m, m, m), (), (0,) * 6, box=16.0 * m / n, order="linear")   # periodic, same cell size as the full level
     assert abs(hb["dx0"] - 1.0 / n) < 1e-15 / n
     ob = np.asarray(hb["origin"]) // 16
-    centre = int(np.where((ob == 1).all(axis=1))[0][0])
-    smax, worst = 0.0, 0.0
-    for p in picks:
+    centre = int(np.where((ob == r).all(axis=1))[0][0])
+    worst = 0.0
+    for p in picks[:nsample]:
         bx, by, bz = (int(x) for x in org[p])
-        o = oracle.Oracle(hb, gamma, nv, threads=8)
-        o.upload(0, wl.split_global(hb, np.ascontiguousarray(block_around(G, bx, by, bz, nb))))
-        smax = max(smax, o.max_speed(0))
-        o.fill_ghosts(0, 0)
-        o.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
-        o.fill_ghosts(0, 1)
-        o.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+        o = oracle.Oracle(hb, gamma, nv, threads=16)
+        o.upload(0, wl.split_global(hb, np.ascontiguousarray(block_around(G, bx, by, bz, nb, r))))
+        for dt in dts:
+            assert dt <= cfl * (1.0 / n) / o.max_speed(0) * (1 + 1e-6)   # the level-wide maximum bounds every sampled block
+            o.advance(cfl, dt)
         O = o.download(0)[centre:centre + 1]
         Gp = g.download(0, int(p), 1).astype(np.float64)
-        worst = max(worst, norm_err(Gp, O, vector=(dtype == "f32")).max())
-    dx = 1.0 / n
-    assert dt <= cfl * dx / smax * (1 + 1e-6)            # the level-wide maximum bounds every sampled block
+        worst = max(worst, norm_err(Gp, O, vector=(dtype == "f32"), label=label).max())
     assert worst <= tol, worst
 
 
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-12), ("f32", 1e-5)])
-def test_config5_stress_512_sampled(gpu, dtype, tol):
+def test_config5_stress_512_sampled_3_steps(gpu, dtype, tol):
     G = wl.stress_global(512, gamma=1.4, seed=20005)
-    check_fullsize(gpu, G, 1.4, 5, dtype, nsample=8, seed=5, tol=tol)
+    check_fullsize(gpu, G, 1.4, 5, dtype, nsample=6, seed=5, tol=tol, steps=3, label="cfg5 512^3 3 steps")
 
 
 @pytest.mark.parametrize("dtype,tol", [("f64", 1e-12), ("f32", 1e-5)])
-def test_config2_kelvin_helmholtz_256_sampled(gpu, dtype, tol):
+def test_config2_kelvin_helmholtz_256_sampled_10_steps(gpu, dtype, tol):
     G = wl.kelvin_helmholtz_global(256, gamma=5.0 / 3.0, seed=20002)
-    check_fullsize(gpu, G, 5.0 / 3.0, 5, dtype, nsample=8, seed=2, tol=tol)
+    check_fullsize(gpu, G, 5.0 / 3.0, 5, dtype, nsample=3, seed=2, tol=tol, steps=10, label="cfg2 256^3 10 steps")
 
 
-def test_config4_mhd_128_sampled(gpu):
+def test_config4_mhd_128_sampled_10_steps(gpu):
     G = wl.mhd_turbulence_global(128, gamma=5.0 / 3.0, seed=20004)
-    check_fullsize(gpu, G, 5.0 / 3.0, 8, "f64", nsample=8, seed=4, tol=1e-12)
+    check_fullsize(gpu, G, 5.0 / 3.0, 8, "f64", nsample=2, seed=4, tol=1e-12, steps=10, label="cfg4 128^3 10 steps")

@@ -323,12 +323,27 @@ def test_config2_kelvin_helmholtz_reduced(gpu, dtype, halo):
     g, o = make_pair(gpu, h, 5.0 / 3.0, 5, dtype, halo=halo)
     upload_both(g, o, wl.split_global(h, wl.kelvin_helmholtz_global(64)), dtype)
     G, O = run_both(g, o, 10, 0.3)
-    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
+    assert norm_err(G, O, vector=(dtype == "f32"), label="cfg2 KH 64^3 10 steps halo=%d" % halo).max() <= TOL[dtype]
+    if dtype == "f32":
+        # S14' in numbers: the strict per-variable error of the GPU is that of plain fp32 arithmetic -- the oracle's own
+        # fp32 instantiation, same scheme, no re-association, run beside its fp64 self on the same data and time steps
+        # (tests/test_oracle_convergence.py pins those numbers on the CPU).  rho v_y (3 % of the vector's maximum) and
+        # rho v_z (0.7 %) sit at 1.1e-5 and 3e-5 in BOTH; every other variable is below 1e-6.
+        import oracle
+        o32 = oracle.Oracle(h, 5.0 / 3.0, 5, bits=32, threads=8)
+        o64 = oracle.Oracle(h, 5.0 / 3.0, 5, threads=8)
+        U0 = wl.split_global(h, wl.kelvin_helmholtz_global(64)).astype(np.float32).astype(np.float64)
+        o32.upload(0, U0); o64.upload(0, U0)
+        for _ in range(10):
+            o32.advance(0.3, o64.advance(0.3))
+        ref, mine = norm_err(o32.download(0), O), norm_err(G, O)
+        assert (mine <= np.maximum(1e-5, 1.5 * ref)).all(), (mine, ref)
 
 
-def test_config3_sedov_amr_5_levels(gpu):
+@pytest.mark.parametrize("halo", [0, 1])
+def test_config3_sedov_amr_5_levels(gpu, halo):
     h = wl.ball_hierarchy(4, 5, bc=(1,) * 6)
-    g, o = make_pair(gpu, h, 1.4, 5)
+    g, o = make_pair(gpu, h, 1.4, 5, halo=halo)
     U = wl.sedov_hierarchy_state(h)
     upload_both(g, o, U, "f64")
     G, O = run_both(g, o, 2, 0.3)
@@ -355,7 +370,7 @@ def test_config5_stress_reduced(gpu, dtype):
     g, o = make_pair(gpu, h, 1.4, 5, dtype, halo=1)
     upload_both(g, o, wl.split_global(h, wl.stress_global(64)), dtype)
     G, O = run_both(g, o, 3, 0.3)
-    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
+    assert norm_err(G, O, vector=(dtype == "f32"), label="cfg5 stress 64^3 3 steps").max() <= TOL[dtype]
 
 
 # ------------------------------------------------------------------ 9-variable GLM-MHD (NEXT-1)
@@ -388,7 +403,7 @@ def test_glm_mhd_turbulence_with_damping(gpu, halo, dtype):
     U = upload_both(g, o, wl.split_global(h, G9), dtype)
     G, O = run_both(g, o, 10, 0.3)
     assert np.abs(O[:, 8]).max() > 1e-3 and np.isfinite(G).all()
-    assert norm_err(G, O, vector=(dtype == "f32")).max() <= TOL[dtype]
+    assert norm_err(G, O, vector=(dtype == "f32"), label="GLM-MHD 32^3 10 steps").max() <= TOL[dtype]
 
 
 def test_glm_amr_two_level(gpu):

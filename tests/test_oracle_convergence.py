@@ -4,7 +4,7 @@ import pytest
 
 import oracle
 from paper_0910_5547_b200 import workloads as wl
-from util import exact_sod, run_to, slab_hierarchy
+from util import exact_sod, norm_err, run_to, slab_hierarchy
 
 
 def _slab_run(nv, gamma, axis, nblk, prim, t_end, cfl, periodic, theta=1.5, ncpu=1):
@@ -99,3 +99,22 @@ def test_p11_alfven_wave_second_order(axis, ncpu):
     assert abs(errs[0] - 8.73e-3) < 0.06 * 8.73e-3, errs
     assert abs(errs[2] - 9.38e-4) < 0.06 * 9.38e-4, errs
     assert o1 > 1.2 and o2 > 1.75, (errs, o1, o2)
+
+
+def test_fp32_arithmetic_bounds_the_strict_per_variable_norm(ncpu):
+    """Why fp32 whole-run parity uses reading S14' for small vector components: the oracle's own fp32 instantiation
+    (same scheme, same operation order, plain fp32) against its fp64 self on config 2 at 64^3, 10 steps, same data
+    and time steps.  rho, rho v_x and E agree to a few 1e-7; rho v_y (3 % of |rho v|_max) and rho v_z (0.7 %) do not
+    reach 1e-5 of their OWN maximum, because the rounding of the O(1) fluxes is absolute.  Measured against the
+    maximum of the momentum vector they are below 1e-6 like everything else."""
+    h = wl.uniform_hierarchy(4, periodic=True)
+    U = wl.split_global(h, wl.kelvin_helmholtz_global(64)).astype(np.float32).astype(np.float64)
+    o64, o32 = oracle.Oracle(h, 5.0 / 3.0, 5, threads=ncpu), oracle.Oracle(h, 5.0 / 3.0, 5, bits=32, threads=ncpu)
+    o64.upload(0, U); o32.upload(0, U)
+    for _ in range(10):
+        o32.advance(0.3, o64.advance(0.3))
+    A, B = o32.download(0), o64.download(0)
+    strict = norm_err(A, B)
+    assert (strict[[0, 1, 4]] < 1e-6).all()
+    assert strict[2] > 5e-6 and strict[3] > 1e-5            # the plain-fp32 scheme itself misses 1e-5 here
+    assert (norm_err(A, B, vector=True) < 1e-6).all()       # S14'

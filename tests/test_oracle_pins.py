@@ -382,3 +382,117 @@ def test_cfl_dt_closed_form():
     G2[:, 7, 20, 3] = wl.cons_from_prim(np.array(2.0), np.array(1.0), (np.array(-2.5), np.array(0.0), np.array(0.0)), g)
     o.upload(0, wl.split_global(h, G2))
     assert abs(o.max_speed(0) - (2.5 + c)) < 1e-14
+
+
+# ------------------------------------------------------------------ P20: the floors of S11, by hand
+def test_p20_primitive_recovery_floors_by_hand():
+    """O1 with the floors of reading S11 (`Phys::prim`): a density below the floor is replaced BEFORE the
+    velocities are formed, an internal energy below the floor AFTER; states above the floors are untouched.
+    Values written out by hand (gamma = 1.4 does not enter O1)."""
+    # rho = 0.5 < 0.8 -> rho := 0.8; v = m / 0.8 = (0.5, -0.25, 1.0); e = E/0.8 - v^2/2 = 4/0.8 - 0.65625 = 4.34375
+    W, hits = oracle.prim_floors(5, 1.4, 0.8, 2.2, [0.5, 0.4, -0.2, 0.8, 4.0])
+    assert hits == 1
+    assert np.array_equal(W, [0.8, 4.34375, 0.5, -0.25, 1.0])
+    # e = 1.0/1.0 - 0.5 (0.25) = 0.875 < 2.2 -> e := 2.2, density and velocities untouched
+    W, hits = oracle.prim_floors(5, 1.4, 0.8, 2.2, [1.0, 0.5, 0.0, 0.0, 1.0])
+    assert hits == 1
+    assert np.array_equal(W, [1.0, 2.2, 0.5, 0.0, 0.0])
+    # both: rho = 0.25 -> 0.8, v = (1, 0, 0), e = 0.4/0.8 - 0.5 = 0 -> 2.2
+    W, hits = oracle.prim_floors(5, 1.4, 0.8, 2.2, [0.25, 0.8, 0.0, 0.0, 0.4])
+    assert hits == 2 and np.array_equal(W, [0.8, 2.2, 1.0, 0.0, 0.0])
+    # negative and NaN densities are floored too (the test is !(rho >= floor)); a state above the floors is untouched
+    assert oracle.prim_floors(5, 1.4, 0.8, 2.2, [-1.0, 0.0, 0.0, 0.0, 8.0])[0][0] == 0.8
+    assert oracle.prim_floors(5, 1.4, 0.8, 2.2, [np.nan, 0.0, 0.0, 0.0, 8.0])[0][0] == 0.8
+    U = [2.0, 1.0, -0.5, 0.25, 12.0]
+    W, hits = oracle.prim_floors(5, 1.4, 0.8, 2.2, U)
+    assert hits == 0 and np.array_equal(W, oracle.prim(5, 1.4, U))
+    assert np.array_equal(W, [2.0, 6.0 - 0.5 * (0.25 + 0.0625 + 0.015625), 0.5, -0.25, 0.125])
+    # MHD: the magnetic energy leaves the energy slot before the floor is tested (PAPER.md:298):
+    # e = (3.0 - 0.5 * 4) / 1 - 0 = 1.0 < 2.2 -> floored; without B the same E would pass (e = 3.0)
+    W, hits = oracle.prim_floors(8, 1.4, 0.8, 2.2, [1.0, 0.0, 0.0, 0.0, 3.0, 2.0, 0.0, 0.0])
+    assert hits == 1 and W[1] == 2.2 and W[5] == 2.0
+    assert oracle.prim_floors(5, 1.4, 0.8, 2.2, [1.0, 0.0, 0.0, 0.0, 3.0]) [1] == 0
+
+
+def test_p20_reconstructed_state_floors_by_hand():
+    """S11 on the l and r states of O2 (`Phys::floor_state` inside `plm`), with theta = 2 so that the limited
+    slope undershoots nowhere by itself: the floors are set ABOVE reconstructed values on purpose.
+    Cells (rho, e, vx, vy, vz): i-2 = (1.0, 3.0), i-1 = (0.9, 2.8), i = (0.7, 2.4), i+1 = (0.6, 2.3), at rest."""
+    cells = [np.array([r, e, 0.0, 0.0, 0.0]) for r, e in ((1.0, 3.0), (0.9, 2.8), (0.7, 2.4), (0.6, 2.3))]
+    # Eq. 9 (G1), theta = 2: rho_l = 0.9 + 0.5 minmod(2(-0.1), 2(-0.2), 0.5(-0.3)) = 0.9 - 0.075 = 0.825
+    #                         e_l  = 2.8 + 0.5 minmod(2(-0.2), 2(-0.4), 0.5(-0.6)) = 2.8 - 0.15  = 2.65
+    # Eq. 10:                 rho_r = 0.7 + 0.5 minmod(2(0.1), 2(0.2), 0.5(0.3))   = 0.7 + 0.075 = 0.775
+    #                         e_r  = 2.4 + 0.5 minmod(2(0.1), 2(0.4), 0.5(0.5))   = 2.4 + 0.1   = 2.5
+    WL, WR, lam, F, hits = oracle.face_floors(5, 1.4, 2.0, 0, 1e-300, 1e-300, *cells)
+    assert hits == 0
+    assert np.allclose([WL[0], WL[1], WR[0], WR[1]], [0.825, 2.65, 0.775, 2.5], rtol=0, atol=2e-16)
+    assert np.array_equal(oracle.face(5, 1.4, 2.0, 0, *cells)[3], F)        # the default helper is the same path
+    # floors between the two states: rho floor 0.8 lifts only rho_r, e floor 2.6 lifts only e_r
+    WL2, WR2, lam2, F2, hits = oracle.face_floors(5, 1.4, 2.0, 0, 0.8, 2.6, *cells)
+    assert hits == 2
+    assert np.array_equal(WL2, WL) and WR2[0] == 0.8 and WR2[1] == 2.6 and np.array_equal(WR2[2:], WR[2:])
+    # Eq. 12 on the floored states, by hand: at rest F_rho = -lam/2 (rho_r - rho_l), F_mx = (p_l + p_r)/2,
+    # lam = max c = sqrt(gamma (gamma - 1) max e) = sqrt(0.56 * 2.65)
+    assert abs(lam2 - np.sqrt(0.56 * 2.65)) < 1e-15
+    assert abs(F2[0] - (-0.5 * lam2 * (0.8 - 0.825))) < 1e-16
+    assert abs(F2[1] - 0.5 * 0.4 * (0.825 * 2.65 + 0.8 * 2.6)) < 1e-15
+    # floors above both states: four activations, both sides equal -> the flux of a uniform state at rest
+    WL3, WR3, lam3, F3, hits = oracle.face_floors(5, 1.4, 2.0, 0, 0.9, 2.7, *cells)
+    assert hits == 4 and WL3[0] == WR3[0] == 0.9 and WL3[1] == WR3[1] == 2.7
+    assert F3[0] == 0.0 and abs(F3[1] - 0.4 * 0.9 * 2.7) < 1e-15 and F3[4] == 0.0
+
+
+def test_p20_floors_fire_inside_a_stage_and_are_counted():
+    """The same floors through `rk_stage` of a hierarchy: one cell below the density floor in otherwise uniform data
+    changes exactly the cells whose stencil (2 cells per side) sees it, and is counted."""
+    h = wl.uniform_hierarchy(1, periodic=True)
+    one = np.ones((1, 16, 16, 16))
+    rho = 1.0 * one
+    rho[0, 8, 8, 8] = 0.5
+    U = np.moveaxis(wl.cons_from_prim(rho, 1.0 * one, (0 * one, 0 * one, 0 * one), 1.4), 0, 1).copy()
+    res = []
+    for fl in (1e-30, 0.8):
+        o = oracle.Oracle(h, 1.4, 5, rho_floor=fl)
+        o.upload(0, U)
+        o.fill_ghosts(0, 0)
+        o.rk_stage(0, 0, 0, 1, 0.0, 1.0, 1e-3)
+        res.append((o.download(1), o.floor_hits()))
+    assert res[0][1] == 0 and res[1][1] > 0
+    diff = np.argwhere(np.abs(res[0][0][0, 0] - res[1][0][0, 0]) > 0)
+    assert len(diff) > 0 and np.abs(diff - 8).max() <= 2          # only the stencil neighbourhood of the cell
+
+
+# ------------------------------------------------------------------ P21: the global time step on a hierarchy (S4)
+def test_p21_global_dt_on_three_levels_closed_form():
+    """`Hier::global_dt` (S4): dt0 = CFL dx0 / max over ALL levels of max(|v_d| + c), and every level l steps with
+    dt0 / 2^l.  Uniform gas at rest (c = sqrt(gamma p / rho) = sqrt(1.4)) with ONE hot, moving cell on level 1:
+    the returned dt must be CFL dx0 / (|v| + c)_hot -- a min for the max, or a per-level dx in place of dx0,
+    would return something else -- and each level's own CFL number dt_l S_l / dx_l stays <= CFL."""
+    lvl1 = [(i, j, k) for i in (1, 2) for j in (1, 2) for k in (1, 2)]
+    lvl2 = [(i, j, k) for i in (3, 4) for j in (3, 4) for k in (3, 4)]
+    h = wl.build_hierarchy((2, 2, 2), [lvl1, lvl2], (0,) * 6)
+    assert h["nlevels"] == 3
+    n = len(h["level"])
+    one = np.ones((n, 16, 16, 16))
+    rho, p = 1.0 * one, 1.0 * one
+    vx, vy, vz = 0 * one, 0 * one, 0 * one
+    hot = int(wl.level_patches(h, 1)[3])
+    p[hot, 5, 6, 7] = 9.0
+    vy[hot, 5, 6, 7] = -2.0
+    U = np.moveaxis(wl.cons_from_prim(rho, p, (vx, vy, vz), 1.4), 0, 1).copy()
+    c0, shot = np.sqrt(1.4), 2.0 + np.sqrt(1.4 * 9.0)
+    dx0 = 1.0 / 32.0
+    for cfl in (0.3, 0.15):
+        o = oracle.Oracle(h, 1.4, 5)
+        o.upload(0, U)
+        assert abs(o.max_speed(0) - c0) < 1e-15 and abs(o.max_speed(2) - c0) < 1e-15
+        assert abs(o.max_speed(1) - shot) < 1e-14
+        dt = o.advance(cfl)
+        assert abs(dt - cfl * dx0 / shot) <= 1e-15 * dt
+        for l, s in enumerate((c0, shot, c0)):
+            assert (dt / 2 ** l) * s / (dx0 / 2 ** l) <= cfl * (1 + 1e-14)
+    # the per-level call uses that level's own dx and maximum (what a single-level run needs)
+    o = oracle.Oracle(h, 1.4, 5)
+    o.upload(0, U)
+    assert abs(o.cfl_dt(2, 0, 0.3) - 0.3 * (dx0 / 4) / c0) < 1e-16
+    assert abs(o.cfl_dt(1, 0, 0.3) - 0.3 * (dx0 / 2) / shot) < 1e-16

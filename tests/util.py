@@ -78,18 +78,32 @@ def run_to(o, t_end, cfl, max_steps=100000):
     return n
 
 
-def norm_err(a, b, vector=False):
-    """S14: per-variable max|a-b| / max|b| (0/0 = 0).  vector=True (used for fp32, reading
-    S14'): the three momentum components, and the three B components, share one scale (the
-    max over the vector), because fp32 rounding of the O(1) fluxes bounds the absolute error
-    of every component alike."""
-    groups = [[v] for v in range(b.shape[1])]
+SMALL_COMPONENT = 0.1      # S14': a vector component whose own max is below this fraction of the vector's max
+FP32_LOG = []              # (label, variable, strict S14 error, norm used, error in that norm): printed by conftest at exit
+
+
+def norm_err(a, b, vector=False, label=None):
+    """S14: per-variable max|a-b| / max|b| (0/0 = 0) -- the norm of BASELINE.json's tolerances.
+    vector=True (fp32 whole-run parity only, reading S14'): a momentum (or B) component whose own maximum is
+    below SMALL_COMPONENT of the largest component of its vector is measured against the vector's maximum
+    instead of its own, because fp32 rounding of the O(1) fluxes bounds the absolute error of every component
+    alike (KH: rho v_z ~ 1e-3 next to rho v_x ~ 1); every other variable keeps the strict per-variable norm.
+    Both numbers are recorded in FP32_LOG (printed at the end of the GPU session)."""
+    nv = b.shape[1]
+    vmax = [float(np.abs(b[:, v]).max()) for v in range(nv)]
+    diff = [float(np.abs(a[:, v] - b[:, v]).max()) for v in range(nv)]
+    scale = list(vmax)
     if vector:
-        groups = [[0], [1, 2, 3], [4]] + ([[5, 6, 7]] if b.shape[1] >= 8 else []) + ([[8]] if b.shape[1] == 9 else [])
+        for grp in ([1, 2, 3],) + (([5, 6, 7],) if nv >= 8 else ()):
+            g = max(vmax[v] for v in grp)
+            for v in grp:
+                if vmax[v] < SMALL_COMPONENT * g:
+                    scale[v] = g
     out = []
-    for grp in groups:
-        s = max(np.abs(b[:, v]).max() for v in grp)
-        for v in grp:
-            d = np.abs(a[:, v] - b[:, v]).max()
-            out.append(0.0 if d == 0 else d / s if s > 0 else np.inf)
+    for v in range(nv):
+        e = 0.0 if diff[v] == 0 else diff[v] / scale[v] if scale[v] > 0 else np.inf
+        out.append(e)
+        if vector:
+            strict = 0.0 if diff[v] == 0 else diff[v] / vmax[v] if vmax[v] > 0 else np.inf
+            FP32_LOG.append((label or "", v, strict, "S14'" if scale[v] != vmax[v] else "S14", e))
     return np.array(out)
