@@ -136,6 +136,24 @@ def ball_hierarchy(base_blocks, nlevels, radius_in_patches=1.5, centre=(0.5, 0.5
     return build_hierarchy(nb, refined, bc, order=order)
 
 
+def blocks_hierarchy(path, base_blocks, bc=(1,) * 6, order="morton"):
+    """Hierarchy from a block list written as text lines "level bx by bz" (levels >= 1; '#' comments).
+    Config 3's criterion-built table (reading S16) is stored this way: tests/golden/cfg3_blocks.txt,
+    written by tests/golden/make_cfg3_hierarchy.py."""
+    nb = (base_blocks,) * 3 if np.isscalar(base_blocks) else tuple(base_blocks)
+    per_level = {}
+    with open(path) as f:
+        for line in f:
+            line = line.split("#")[0].split()
+            if not line:
+                continue
+            l, bx, by, bz = (int(x) for x in line)
+            per_level.setdefault(l, []).append((bx, by, bz))
+    nlev = max(per_level) if per_level else 0
+    refined = [per_level.get(l, []) for l in range(1, nlev + 1)]
+    return build_hierarchy(nb, refined, bc, order=order)
+
+
 def level_patches(h, l):
     return np.nonzero(h["level"] == l)[0]
 

@@ -1,5 +1,7 @@
 """GPU parity: every C-ABI call against the CPU oracle, element by element, on the same seeded
 inputs (norm S14; tolerances 1e-12 fp64, 1e-5 fp32 from BASELINE.json)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -341,7 +343,8 @@ def test_config2_kelvin_helmholtz_reduced(gpu, dtype, halo):
 
 
 @pytest.mark.parametrize("halo", [0, 1])
-def test_config3_sedov_amr_5_levels(gpu, halo):
+def test_sedov_amr_5_levels_nested_balls(gpu, halo):
+    """Config 3's state on the nested-ball stand-in hierarchy (288 patches; kept as a smaller unit case)."""
     h = wl.ball_hierarchy(4, 5, bc=(1,) * 6)
     g, o = make_pair(gpu, h, 1.4, 5, halo=halo)
     U = wl.sedov_hierarchy_state(h)
@@ -350,6 +353,46 @@ def test_config3_sedov_amr_5_levels(gpu, halo):
     assert np.isfinite(G).all()
     assert norm_err(G, O).max() <= 1e-12
     # composite conservation on the GPU: level-0 sums (covered cells hold restricted data)
+    l0 = wl.level_patches(h, 0)
+    tot0 = U[l0].sum(axis=(0, 2, 3, 4)); tot1 = G[l0].sum(axis=(0, 2, 3, 4))
+    assert abs(tot1[0] - tot0[0]) <= 1e-13 * tot0[0]
+
+
+_CFG3 = {}
+
+
+def cfg3_oracle_run():
+    """Config 3 on its criterion-built hierarchy (reading S16: tests/golden/cfg3_blocks.txt, written by
+    tests/golden/make_cfg3_hierarchy.py from the oracle alone): 64 + 64 + 160 + 432 + 1880 patches, 2 coarse steps
+    (= 32 finest substeps, the parity length of SURVEY 8(d)).  The oracle runs once for both halo modes."""
+    if not _CFG3:
+        import oracle
+        h = wl.blocks_hierarchy(os.path.join(os.path.dirname(__file__), "golden", "cfg3_blocks.txt"), 4)
+        assert [int((h["level"] == l).sum()) for l in range(5)] == [64, 64, 160, 432, 1880]
+        U = wl.sedov_hierarchy_state(h)
+        o = oracle.Oracle(h, 1.4, 5, threads=os.cpu_count() or 1)
+        o.upload(0, U)
+        dts = [o.advance(0.3) for _ in range(2)]
+        assert o.floor_hits() == 0
+        _CFG3.update(h=h, U=U, O=o.download(0), dts=dts)
+    return _CFG3
+
+
+@pytest.mark.parametrize("halo", [0, 1])
+def test_config3_sedov_amr_criterion_built_hierarchy(gpu, halo):
+    c = cfg3_oracle_run()
+    h, U, O = c["h"], c["U"], c["O"]
+    g = gpu.AmrHydro(h, 1.4, 5, halo=halo)
+    g.upload(0, U)
+    dts = [g.advance(0.3) for _ in range(2)]
+    assert all(abs(a - b) <= 1e-12 * b for a, b in zip(dts, c["dts"]))
+    G = g.download(0)
+    assert np.isfinite(G).all() and g.get_counter(gpu.CNT_FLOOR_HITS) == 0
+    assert norm_err(G, O).max() <= 1e-12
+    # per level too: a level's own maximum is its scale (the ambient levels must not hide behind the blast)
+    for l in range(h["nlevels"]):
+        ps = wl.level_patches(h, l)
+        assert norm_err(G[ps], O[ps]).max() <= 1e-12, l
     l0 = wl.level_patches(h, 0)
     tot0 = U[l0].sum(axis=(0, 2, 3, 4)); tot1 = G[l0].sum(axis=(0, 2, 3, 4))
     assert abs(tot1[0] - tot0[0]) <= 1e-13 * tot0[0]

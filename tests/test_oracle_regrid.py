@@ -106,3 +106,25 @@ def test_p19_prolongation_is_conservative_exact_on_linear_data_and_monotone():
         assert (k >= up(lo) - 1e-15).all() and (k <= up(hi) + 1e-15).all()
     with pytest.raises(ValueError):
         o.prolong_interior(0)                                  # a level-0 patch has no parent
+
+
+# ---------------------------------------------------------------- S16: config 3's hierarchy by its own criterion
+def test_cfg3_blocks_golden_is_what_the_script_writes(tmp_path, monkeypatch):
+    """tests/golden/cfg3_blocks.txt is reproduced from the oracle alone by the committed script, is properly
+    nested (build_hierarchy checks it), holds the deposit on its finest level and has the counts DESIGN.md states."""
+    import importlib.util
+    import os
+    gold = os.path.join(os.path.dirname(__file__), "golden")
+    spec = importlib.util.spec_from_file_location("make_cfg3_hierarchy", os.path.join(gold, "make_cfg3_hierarchy.py"))
+    m = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(m)
+    monkeypatch.setattr(m, "HERE", str(tmp_path))
+    m.main()
+    body = lambda p: [ln for ln in open(p).read().splitlines() if ln and not ln.startswith("#")]
+    assert body(os.path.join(str(tmp_path), "cfg3_blocks.txt")) == body(os.path.join(gold, "cfg3_blocks.txt"))
+    h = wl.blocks_hierarchy(os.path.join(gold, "cfg3_blocks.txt"), 4)
+    assert [int((h["level"] == l).sum()) for l in range(5)] == [64, 64, 160, 432, 1880]
+    U = wl.sedov_hierarchy_state(h)
+    l4 = wl.level_patches(h, 4)
+    dx4 = h["dx0"] / 16
+    assert abs((U[l4, 4] - 1e-5 / 0.4).sum() * dx4 ** 3 - 1.0) <= 1e-12        # E = 1 on the finest level
