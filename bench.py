@@ -48,8 +48,10 @@ def parse():
     ap.add_argument("--kernel", type=int, default=3, help="3 = k_rk_stage_pair (nvars = 5; k_rk_stage_march otherwise), 2 = k_rk_stage_march, 0 = reference")
     ap.add_argument("--zsplit", type=int, default=2, help="AMRHYDRO_OPT_ZSPLIT (2 = automatic)")
     ap.add_argument("--fuse-cfl", type=int, default=2, help="AMRHYDRO_OPT_FUSE_CFL (2 = library default)")
+    ap.add_argument("--graph", type=int, default=1, help="AMRHYDRO_OPT_GRAPH for the AMR workload (cfg3): one CUDA-graph replay per coarse step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-fp32", action="store_true", help="skip the fp32 sub-record of the default fp64 run (cfg5, cfg2)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     return ap.parse_args()
 
@@ -235,7 +237,8 @@ def run_ours(args):
     single = h["nlevels"] == 1
     esz = 8 if args.dtype == "f64" else 4
     npdt = np.float64 if args.dtype == "f64" else np.float32
-    g = binding.AmrHydro(h, gamma, nv, dtype=args.dtype, halo=args.halo, kernel=args.kernel, zsplit=args.zsplit, fuse_cfl=args.fuse_cfl, device="cuda:%d" % local)
+    g = binding.AmrHydro(h, gamma, nv, dtype=args.dtype, halo=args.halo, kernel=args.kernel, zsplit=args.zsplit, fuse_cfl=args.fuse_cfl,
+                         graph=0 if single else args.graph, device="cuda:%d" % local)
     host_in = torch.empty((npatch, nv, 16, 16, 16), dtype=torch.float64 if esz == 8 else torch.float32, pin_memory=True)
     host_in.numpy()[...] = U.astype(npdt, copy=False)
     del U
@@ -243,27 +246,6 @@ def run_ours(args):
     g.sync()
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    stage_ev = []
-
-    def step(record=False):
-        if single:
-            dt = g.cfl_dt(0, 0, cfl)
-            g.fill_ghosts(0, 0)
-            if record:
-                e0, e1, e2, e3 = ev(), ev(), ev(), ev()
-                e0.record()
-            g.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
-            if record:
-                e1.record()
-            g.fill_ghosts(0, 1)
-            if record:
-                e2.record()
-            g.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
-            if record:
-                e3.record()
-                stage_ev.append((e0, e1, e2, e3))
-        else:
-            g.advance(cfl)
 
     def barrier():
         torch.cuda.synchronize()
@@ -271,61 +253,111 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(max(3, args.warmup)):
-        step()
-    barrier()
-    g.get_counter(binding.CNT_LAUNCHES, reset=True)
-    sampler = ClockSampler(local) if rank == 0 else None
-    t0, t1 = ev(), ev()
-    t0.record()
-    for _ in range(args.steps):
-        step(record=True)
-    t1.record()
-    barrier()
-    ms = t0.elapsed_time(t1)
-    clocks = sampler.stop() if sampler else {}
-    launches = g.get_counter(binding.CNT_LAUNCHES)
-    ms = max_over_ranks(ms, dist, "cuda")
-    ms_per_step = ms / args.steps
-    value = whole_job_rate(upd_per_step, world, args.steps, ms)
+    def measure(g, dtype):
+        """W warm-up steps, then K timed steps (CUDA events on the library's stream = torch's current stream, barrier +
+        synchronize on both sides, max over ranks); per-stage events inside the timed region for the roofline."""
+        esz = 8 if dtype == "f64" else 4
+        stage_ev = []
 
-    # finiteness of the state after the timed run (S4 warning): sample the first patches
-    chk = g.download(0, 0, min(npatch, 64))
-    finite = bool(np.isfinite(chk).all())
+        def step(record=False):
+            if single:
+                dt = g.cfl_dt(0, 0, cfl)
+                g.fill_ghosts(0, 0)
+                if record:
+                    e0, e1, e2, e3 = ev(), ev(), ev(), ev()
+                    e0.record()
+                g.rk_stage(0, 0, 0, 1, 0.0, 1.0, dt)
+                if record:
+                    e1.record()
+                g.fill_ghosts(0, 1)
+                if record:
+                    e2.record()
+                g.rk_stage(0, 1, 0, 0, 0.5, 0.5, dt)
+                if record:
+                    e3.record()
+                    stage_ev.append((e0, e1, e2, e3))
+            else:
+                g.advance(cfl, want_dt=False)          # (no host read of dt: with the graph the step does not synchronise)
 
-    # roofline of the dominant kernel (rk_stage): algorithmic bytes / measured launch time
-    peak, peak_src = peaks()
-    roof = None
-    if stage_ev:
-        s1 = float(np.mean([a.elapsed_time(b) for a, b, _, _ in stage_ev]))
-        s2 = float(np.mean([c.elapsed_time(d) for _, _, c, d in stage_ev]))
-        cells = npatch * 4096
-        b1, b2 = 2 * nv * esz * cells, 3 * nv * esz * cells       # stage 1: read U write U1; stage 2: + read Un
-        avg_ms = 0.5 * (s1 + s2)
-        ach = 0.5 * (b1 + b2) / (avg_ms * 1e-3) / 1e9
-        key = "%s_%s" % (args.workload, args.dtype)
-        roof = {"bound": "hbm", "kernel": {0: "k_rk_stage_ref", 2: "k_rk_stage_march", 3: "k_rk_stage_pair" if nv == 5 else "k_rk_stage_march"}[args.kernel],
-                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": NCU_TRAFFIC.get(key), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": 0.5 * (b1 + b2),
-                "stage1": {"ms": s1, "GB/s": b1 / (s1 * 1e-3) / 1e9, "bytes_per_cell": 2 * nv * esz},
-                "stage2": {"ms": s2, "GB/s": b2 / (s2 * 1e-3) / 1e9, "bytes_per_cell": 3 * nv * esz},
-                "share_of_step": (s1 + s2) / ms_per_step,
-                "frac_of_nominal_8TBs": ach / 8000.0}
-        # the arithmetic side of the same kernel: executed thread-instructions
-        # per cell and stage from the committed ncu capture / the SM's issue and FP64-pipe rates
-        ipc = (NCU_TRAFFIC.get("instr_per_cell_stage") or {}).get(key)
-        if ipc:
-            clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
-            alu = {"bound": "alu", "unit": "G thread-instr/s", "sm_mhz": clk / 1e6,
-                   "issue": {"instr_per_cell_stage": ipc["total"], "achieved": ipc["total"] * cells / (avg_ms * 1e-3) / 1e9,
-                             "peak": 148 * 128 * clk / 1e9}}
-            alu["issue"]["frac"] = alu["issue"]["achieved"] / alu["issue"]["peak"]
-            if "fp64" in ipc:
-                alu["fp64_pipe"] = {"instr_per_cell_stage": ipc["fp64"], "achieved": ipc["fp64"] * cells / (avg_ms * 1e-3) / 1e9,
-                                    "peak": 148 * 64 * clk / 1e9}
-                alu["fp64_pipe"]["frac"] = alu["fp64_pipe"]["achieved"] / alu["fp64_pipe"]["peak"]
-            roof["alu"] = alu
+        for _ in range(max(3, args.warmup)):
+            step()
+        barrier()
+        g.get_counter(binding.CNT_LAUNCHES, reset=True)
+        sampler = ClockSampler(local) if rank == 0 else None
+        t0, t1 = ev(), ev()
+        t0.record()
+        for _ in range(args.steps):
+            step(record=True)
+        t1.record()
+        barrier()
+        ms = t0.elapsed_time(t1)
+        clocks = sampler.stop() if sampler else {}
+        launches = g.get_counter(binding.CNT_LAUNCHES)
+        ms = max_over_ranks(ms, dist, "cuda")
+        ms_per_step = ms / args.steps
+        value = whole_job_rate(upd_per_step, world, args.steps, ms)
+
+        # finiteness of the state after the timed run (S4 warning): sample the first patches
+        chk = g.download(0, 0, min(npatch, 64))
+        finite = bool(np.isfinite(chk).all())
+
+        # roofline of the dominant kernel (rk_stage): algorithmic bytes / measured launch time
+        peak, peak_src = peaks()
+        roof = None
+        if stage_ev:
+            s1 = float(np.mean([a.elapsed_time(b) for a, b, _, _ in stage_ev]))
+            s2 = float(np.mean([c.elapsed_time(d) for _, _, c, d in stage_ev]))
+            cells = npatch * 4096
+            b1, b2 = 2 * nv * esz * cells, 3 * nv * esz * cells       # stage 1: read U write U1; stage 2: + read Un
+            avg_ms = 0.5 * (s1 + s2)
+            ach = 0.5 * (b1 + b2) / (avg_ms * 1e-3) / 1e9
+            key = "%s_%s" % (args.workload, dtype)
+            traffic = NCU_TRAFFIC.get(key)
+            roof = {"bound": "hbm", "kernel": {0: "k_rk_stage_ref", 2: "k_rk_stage_march", 3: "k_rk_stage_pair" if nv == 5 else "k_rk_stage_march"}[args.kernel],
+                    "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": traffic, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": 0.5 * (b1 + b2),
+                    # the same launches in real DRAM bytes (ncu dram__bytes_read + write per launch, profiles/traffic.json)
+                    "dram_frac": (traffic / (avg_ms * 1e-3) / 1e9 / peak) if traffic else None,
+                    "stage1": {"ms": s1, "GB/s": b1 / (s1 * 1e-3) / 1e9, "bytes_per_cell": 2 * nv * esz},
+                    "stage2": {"ms": s2, "GB/s": b2 / (s2 * 1e-3) / 1e9, "bytes_per_cell": 3 * nv * esz},
+                    "share_of_step": (s1 + s2) / ms_per_step,
+                    "frac_of_nominal_8TBs": ach / 8000.0}
+            # the arithmetic side of the same kernel (DESIGN.md section 5): executed thread-instructions
+            # per cell and stage from the committed ncu capture / the SM's issue and FP64-pipe rates
+            ipc = (NCU_TRAFFIC.get("instr_per_cell_stage") or {}).get(key)
+            if ipc:
+                clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
+                alu = {"bound": "alu", "unit": "G thread-instr/s", "sm_mhz": clk / 1e6,
+                       "issue": {"instr_per_cell_stage": ipc["total"], "achieved": ipc["total"] * cells / (avg_ms * 1e-3) / 1e9,
+                                 "peak": 148 * 128 * clk / 1e9}}
+                alu["issue"]["frac"] = alu["issue"]["achieved"] / alu["issue"]["peak"]
+                if "fp64" in ipc:
+                    alu["fp64_pipe"] = {"instr_per_cell_stage": ipc["fp64"], "achieved": ipc["fp64"] * cells / (avg_ms * 1e-3) / 1e9,
+                                        "peak": 148 * 64 * clk / 1e9}
+                    alu["fp64_pipe"]["frac"] = alu["fp64_pipe"]["achieved"] / alu["fp64_pipe"]["peak"]
+                roof["alu"] = alu
+        return dict(value=value, ms_per_step=ms_per_step, roofline=roof, clocks=clocks, launches=int(launches), finite=finite)
+
+    m = measure(g, args.dtype)
+    value, ms_per_step, roof, clocks, launches, finite = (m[k] for k in ("value", "ms_per_step", "roofline", "clocks", "launches", "finite"))
+
+    # the other precision the configuration names (BASELINE.json configs[1] and [4]: "run in fp32 and fp64"): the same
+    # workload, steps and timing rules in fp32, reported as a sub-record; the top-level value stays fp64
+    fp32 = None
+    if args.dtype == "f64" and args.workload in ("cfg5", "cfg2") and not args.no_fp32:
+        g32 = binding.AmrHydro(h, gamma, nv, dtype="f32", halo=args.halo, kernel=args.kernel, zsplit=args.zsplit, fuse_cfl=args.fuse_cfl, device="cuda:%d" % local)
+        h32 = torch.empty((npatch, nv, 16, 16, 16), dtype=torch.float32, pin_memory=True)
+        h32.numpy()[...] = host_in.numpy()
+        g32.upload_ptr(0, 0, npatch, h32.data_ptr())
+        g32.sync()
+        m32 = measure(g32, "f32")
+        fp32 = {"value": m32["value"], "unit": "cell-updates/s", "ms_per_step": m32["ms_per_step"], "dtype": "f32",
+                "roofline": m32["roofline"], "clocks": m32["clocks"], "gpu_launches": m32["launches"], "finite": m32["finite"]}
+        finite = finite and m32["finite"]
+        launches += m32["launches"]
+        del g32, h32
+        torch.cuda.empty_cache()
 
     # end to end through the C ABI with host buffers (H2D of all interiors, one step, D2H)
     e2e = None
@@ -361,8 +393,9 @@ def run_ours(args):
                        "cfl": cfl, "halo": "direct sibling reads" if args.halo else "materialised ghosts",
                        "l2_policy": "working set (%.1f GB per slot) far exceeds the 126 MB L2" % (npatch * nv * 4096 * esz / 1e9)
                        if npatch * nv * 4096 * esz > 4 * 126e6 else "working set fits L2 (small config)",
-                       "parallelism": "replicas, one per GPU" if world > 1 else "single GPU"},
-            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                       "parallelism": "replicas, one per GPU" if world > 1 else "single GPU",
+                       **({} if single else {"cuda_graph": bool(args.graph), "graph_replays": int(g.get_counter(binding.CNT_GRAPH_REPLAYS))})},
+            "roofline": roof, "fp32": fp32, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
             "clocks": clocks, "finite": finite,
             "paper_context": "paper reports 8-10x vs one 3 GHz core on a Quadro FX 5600, fp32 (PAPER.md:274)",
         }

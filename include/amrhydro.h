@@ -69,9 +69,17 @@ extern "C" {
                                      (3 warm-up planes more per CTA, about half the latency of a launch):
                                      0 = never, 1 = always, 2 (default) = on levels of at most SMs/2 patches; any time */
 
+#define AMRHYDRO_OPT_GRAPH 11      /* amrhydro_advance replays one CUDA graph per coarse step (dt may stay in
+                                     device memory for graph capture): the S9 recursion is captured once per hierarchy
+                                     and option set, dt0 = cfl dx0 / max_l S_max,l (S4) is formed on the device by k_dt0
+                                     and read by the captured launches, so the host does not wait for dt.  Results are
+                                     bitwise those of the eager path.  0 (default) = eager launches, 1 = graph from the
+                                     second step on; the 9-variable system with psi damping stays eager; any time   */
+
 /* counters (amrhydro_get_counter) */
 #define AMRHYDRO_CNT_LAUNCHES 1   /* kernels launched by this handle since create / last reset */
 #define AMRHYDRO_CNT_FLOOR_HITS 2 /* cells/states where a floor of S11 was applied (rk_stage, cfl) */
+#define AMRHYDRO_CNT_GRAPH_REPLAYS 3 /* coarse steps amrhydro_advance ran as a graph replay (AMRHYDRO_OPT_GRAPH) */
 
 #define AMRHYDRO_BC_PERIODIC 0    /* handled by the neighbour table */
 #define AMRHYDRO_BC_OUTFLOW 1     /* zero-gradient (S5)             */
@@ -178,7 +186,10 @@ int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor);
 
 /* Host-side driver (bookkeeping only): one coarse step of the whole hierarchy with
  * ratio-2 subcycling (S9), slots 0/1/2 as above.  dt_fixed > 0 overrides the CFL step
- * dt0 = cfl*dx0 / max_l S_max,l (S4).  Synchronises once (for dt) unless dt_fixed > 0. */
+ * dt0 = cfl*dx0 / max_l S_max,l (S4).  Synchronises once (for dt) unless dt_fixed > 0.
+ * With AMRHYDRO_OPT_GRAPH = 1 the step is a graph replay that takes dt0 from device memory: dt_out may then be
+ * NULL, in which case the call does not synchronise at all (a zero / non-finite signal speed is reported by the next
+ * call that passes dt_out, as AMRHYDRO_ENONFINITE). */
 int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out);
 /* End-to-end variant with host buffers: upload all interiors into slot 0, `nsteps` coarse
  * steps, download slot 0.  host_in/host_out: [npatches][var][16][16][16]. */

@@ -13,8 +13,8 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 # AMRHYDRO_LIB: an alternative build of the same library (kernel tuning variants)
 _SO = os.environ.get("AMRHYDRO_LIB") or os.path.join(_DIR, "libamrhydro.so")
 
-OPT_DTYPE, OPT_THETA, OPT_RHO_FLOOR, OPT_EINT_FLOOR, OPT_KERNEL, OPT_HALO, OPT_FUSE_CFL, OPT_GLM_CH, OPT_GLM_CR, OPT_ZSPLIT = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
-CNT_LAUNCHES, CNT_FLOOR_HITS = 1, 2
+OPT_DTYPE, OPT_THETA, OPT_RHO_FLOOR, OPT_EINT_FLOOR, OPT_KERNEL, OPT_HALO, OPT_FUSE_CFL, OPT_GLM_CH, OPT_GLM_CR, OPT_ZSPLIT, OPT_GRAPH = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
+CNT_LAUNCHES, CNT_FLOOR_HITS, CNT_GRAPH_REPLAYS = 1, 2, 3
 
 EXPORTS = [
     "amrhydro_create", "amrhydro_destroy", "amrhydro_last_error", "amrhydro_set_option",
@@ -83,7 +83,7 @@ class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
     def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=3, halo=1,
-                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2):
+                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2, graph=0):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():
             raise AmrHydroError("no CUDA device: the amrhydro path has no CPU fallback")
@@ -98,7 +98,7 @@ class AmrHydro:
         self.np_dtype = {"f64": np.float64, "f32": np.float32}[dtype]
         self._ok(self.L.amrhydro_set_option(self.h, OPT_DTYPE, 64.0 if dtype == "f64" else 32.0))
         for k, v in ((OPT_THETA, theta), (OPT_RHO_FLOOR, rho_floor), (OPT_EINT_FLOOR, e_floor),
-                     (OPT_KERNEL, kernel), (OPT_HALO, halo), (OPT_FUSE_CFL, fuse_cfl), (OPT_ZSPLIT, zsplit)) + \
+                     (OPT_KERNEL, kernel), (OPT_HALO, halo), (OPT_FUSE_CFL, fuse_cfl), (OPT_ZSPLIT, zsplit), (OPT_GRAPH, graph)) + \
                 (((OPT_GLM_CH, ch), (OPT_GLM_CR, cr)) if nvars == 9 else ()):
             self._ok(self.L.amrhydro_set_option(self.h, k, float(v)))
         self.hier = hier
@@ -207,7 +207,11 @@ class AmrHydro:
     def copy_slot(self, level, src, dst):
         self._ok(self.L.amrhydro_copy_slot(self.h, level, src, dst))
 
-    def advance(self, cfl, dt=0.0):
+    def advance(self, cfl, dt=0.0, want_dt=True):
+        """want_dt=False passes dt_out = NULL: with graph=1 the call then does not synchronise."""
+        if not want_dt:
+            self._ok(self.L.amrhydro_advance(self.h, cfl, dt, None))
+            return None
         out = C.c_double(0)
         self._ok(self.L.amrhydro_advance(self.h, cfl, dt, C.byref(out)))
         return out.value

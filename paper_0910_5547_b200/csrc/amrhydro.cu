@@ -53,6 +53,18 @@ struct amrhydro {
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
   long long launches = 0;
+  // amrhydro_advance as one CUDA graph (AMRHYDRO_OPT_GRAPH): dt0 lives in d_dt, the S9 recursion is captured once per
+  // hierarchy / option set and replayed; the host-side bookkeeping a replay skips is restored from the capture
+  int use_graph = 0;
+  double *d_dt = nullptr;                   // [0] dt0, [1] non-finite flag (k_dt0)
+  bool dt_dev = false;                      // launches take dt from d_dt (set while capturing)
+  cudaStream_t cap_stream = nullptr;        // capture runs on a stream of the handle's own (the caller's may be the legacy
+                                            // default stream, which cannot be captured); replays go to the caller's stream
+  cudaGraphExec_t graph_exec = nullptr;
+  bool graph_valid = false;
+  std::vector<int> graph_smax_slot;
+  long long graph_launches = 0;
+  long long eager_steps = 0, graph_replays = 0;
   CUtensorMap tmap;            // TMA view of the pool, 16x16 boxes (rk_stage_march, rk_stage_pair)
   bool have_tmap = false;
   std::string err;
@@ -134,7 +146,14 @@ void smax_touch(amrhydro *h, int level, int slot) {
   if (level >= 0 && level < (int)h->smax_slot.size() && h->smax_slot[level] == slot) h->smax_slot[level] = -1;
 }
 
+void drop_graph(amrhydro *h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  h->graph_exec = nullptr;
+  h->graph_valid = false;
+}
+
 void free_hierarchy(amrhydro *h) {
+  drop_graph(h);
   cudaFree(h->d_desc); cudaFree(h->d_child); cudaFree(h->d_octant);
   cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux); cudaFree(h->d_smax);
   h->d_smax = nullptr;
@@ -164,7 +183,9 @@ amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) 
       h->num_sms = sms;
   }
   if (cudaMalloc(&h->d_scalars, 2 * sizeof(unsigned long long)) != cudaSuccess) { delete h; return nullptr; }
+  if (cudaMalloc(&h->d_dt, 2 * sizeof(double)) != cudaSuccess) { cudaFree(h->d_scalars); delete h; return nullptr; }
   cudaMemset(h->d_scalars, 0, 2 * sizeof(unsigned long long));
+  cudaMemset(h->d_dt, 0, 2 * sizeof(double));
   cudaDeviceSynchronize();                 // (legacy-stream memset; later work runs on the caller's stream)
   return h;
 }
@@ -174,6 +195,8 @@ void amrhydro_destroy(amrhydro_t *h) {
   if (h->bound) cudaStreamSynchronize(h->stream);
   free_hierarchy(h);
   cudaFree(h->d_scalars);
+  cudaFree(h->d_dt);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   cudaFree(h->d_stage);
   delete h;
 }
@@ -182,7 +205,13 @@ const char *amrhydro_last_error(const amrhydro_t *h) { return h ? h->err.c_str()
 
 int amrhydro_set_option(amrhydro_t *h, int key, double value) {
   if (!h) return AMRHYDRO_EINVAL;
+  if (h->bound && h->graph_valid) cudaStreamSynchronize(h->stream);
+  drop_graph(h);                              // every option is baked into the captured launches
   switch (key) {
+    case AMRHYDRO_OPT_GRAPH:
+      if (value != 0 && value != 1) return fail(h, AMRHYDRO_EINVAL, "graph must be 0 or 1");
+      h->use_graph = int(value);
+      return 0;
     case AMRHYDRO_OPT_DTYPE:
       if (h->bound) return fail(h, AMRHYDRO_ESTATE, "dtype must be set before bind_pool");
       if (value != 32 && value != 64) return fail(h, AMRHYDRO_EINVAL, "dtype must be 32 or 64");
@@ -233,6 +262,11 @@ int amrhydro_get_counter(amrhydro_t *h, int key, long long *out, int reset) {
     if (reset) h->launches = 0;
     return 0;
   }
+  if (key == AMRHYDRO_CNT_GRAPH_REPLAYS) {
+    *out = h->graph_replays;
+    if (reset) h->graph_replays = 0;
+    return 0;
+  }
   if (key == AMRHYDRO_CNT_FLOOR_HITS) {
     unsigned long long v = 0;
     CUDA_TRY(h, cudaMemcpyAsync(&v, h->d_scalars + 1, sizeof(v), cudaMemcpyDeviceToHost, h->stream));
@@ -255,6 +289,7 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   if (need == 0) return fail(h, AMRHYDRO_EINVAL, "bad max_patches / nslots");
   if (bytes < need) return fail(h, AMRHYDRO_ENOMEM, "pool smaller than amrhydro_pool_bytes()");
   if ((uintptr_t)dev_pool % 256) return fail(h, AMRHYDRO_EINVAL, "pool must be 256-byte aligned");
+  drop_graph(h);
   h->pool = dev_pool; h->pool_bytes = bytes; h->maxp = max_patches; h->nslots = nslots;
   h->stream = (cudaStream_t)stream;
   h->bound = true;
@@ -560,6 +595,8 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     constexpr int NV = decltype(nv)::value;
     const int n = h->lev_count[level], first = h->lev_first[level];
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
+    // captured step: dt carries the exact factor 2^-level and the launches read dt0 from device memory
+    const DtDev dtd = h->dt_dev ? DtDev{h->d_dt, dt, hx} : DtDev{nullptr, 0.0, 0.0};
     smax_touch(h, level, sout);
     // the combination stage can also reduce the max signal speed of what it writes (a1 fused into a6)
     const bool fuse = h->kernel != 0 && h->fuse_cfl != 0 && a != 0.0;
@@ -567,27 +604,27 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
-                                                                T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1);
+                                                                T(dt / hx), make_params<T>(h), bflux, h->d_scalars + 1, dtd);
       LAUNCH_CHECK(h);
     } else if (h->kernel == 3 && NV == 5) {
       if constexpr (NV == 5) {
         int r = launch_rk_stage_pair<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                             make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                            fuse ? h->d_smax + level : nullptr, zs);
+                                            fuse ? h->d_smax + level : nullptr, zs, dtd);
         if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_pair: ") + cudaGetErrorString((cudaError_t)r));
         LAUNCH_CHECK(h);
       }
     } else {
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                           fuse ? h->d_smax + level : nullptr, zs);
+                                           fuse ? h->d_smax + level : nullptr, zs, dtd);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
     }
     if (fuse) h->smax_slot[level] = sout;
     if (regs) {
       k_flux_registers<T, NV><<<dim3(n, 54), 64, 0, h->stream>>>(first, level, h->d_desc, h->d_child, bflux,
-                                                                  (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt));
+                                                                  (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt), w, dtd);
       LAUNCH_CHECK(h);
     }
     return 0;
@@ -717,9 +754,61 @@ static int advance_level(amrhydro_t *h, int lev, double dt, double a1, double a2
   return 0;
 }
 
+// One coarse step as a graph replay: the per-level maxima are brought up to date eagerly (k_cfl only where no fused
+// reduction left a valid value), k_dt0 turns them into dt0 in device memory, and the captured S9 recursion reads it.
+static int advance_graph(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out) {
+  if (!(dt_fixed > 0.0))
+    for (int l = 0; l < h->nlev; ++l)
+      if (int r = ensure_smax(h, l, 0)) return r;
+  k_dt0<<<1, 32, 0, h->stream>>>(h->d_smax, 0, h->nlev - 1, cfl * h->dx0, dt_fixed, h->d_dt);
+  LAUNCH_CHECK(h);
+  if (!h->graph_valid) {
+    const std::vector<int> keep = h->smax_slot;
+    const long long l0 = h->launches;
+    cudaGraph_t g = nullptr;
+    if (!h->cap_stream) CUDA_TRY(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    CUDA_TRY(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    h->stream = h->cap_stream;
+    h->dt_dev = true;
+    const int r = advance_level(h, 0, 1.0, 0.0, 0.0);          // "dt" = the factor 2^-level
+    h->dt_dev = false;
+    h->stream = user;
+    const cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    h->graph_smax_slot = h->smax_slot;
+    h->graph_launches = h->launches - l0;
+    h->smax_slot = keep;
+    h->launches = l0;
+    if (r || e != cudaSuccess || !g) {
+      if (g) cudaGraphDestroy(g);
+      cudaGetLastError();
+      return r ? r : fail(h, AMRHYDRO_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+    }
+    const cudaError_t e2 = cudaGraphInstantiate(&h->graph_exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e2 != cudaSuccess) { h->graph_exec = nullptr; return fail(h, AMRHYDRO_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e2)); }
+    h->graph_valid = true;
+  }
+  CUDA_TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
+  h->smax_slot = h->graph_smax_slot;
+  h->launches += h->graph_launches;
+  ++h->graph_replays;
+  if (dt_out) {
+    double v[2] = {0, 0};
+    CUDA_TRY(h, cudaMemcpyAsync(v, h->d_dt, sizeof(v), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    *dt_out = v[0];
+    if (v[1] != 0.0) return fail(h, AMRHYDRO_ENONFINITE, "max signal speed is zero or not finite");
+  }
+  return 0;
+}
+
 int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out) {
   if (int r = check_ready(h)) return r;
   if (h->nslots < (h->nlev > 1 ? 3 : 2)) return fail(h, AMRHYDRO_ESTATE, "advance needs 2 slots (3 with refinement)");
+  // graph replay from the second step on (the first one runs eagerly: it configures the kernels); the GLM damping factor
+  // exp(-dt c_h / c_r) is a host value, so the 9-variable system with damping stays eager
+  if (h->use_graph && h->eager_steps > 0 && !(h->nv == 9 && h->glm_cr > 0.0)) return advance_graph(h, cfl, dt_fixed, dt_out);
   double dt = dt_fixed;
   if (!(dt > 0.0)) {
     for (int l = 0; l < h->nlev; ++l)
@@ -729,6 +818,7 @@ int amrhydro_advance(amrhydro_t *h, double cfl, double dt_fixed, double *dt_out)
     dt = cfl * h->dx0 / s;                                  // S4: dt_l = dt0 / 2^l
   }
   if (dt_out) *dt_out = dt;
+  ++h->eager_steps;
   return advance_level(h, 0, dt, 0.0, 0.0);
 }
 

@@ -92,6 +92,22 @@ __global__ void __launch_bounds__(256) k_cfl(Pool<T> pool, int slot, int first, 
   if (hits) atomicAdd(floor_hits, (unsigned long long)hits);
 }
 
+// S4 on the device: dt0 = cfl_dx0 / max_l S_max,l from the per-level maxima (bit patterns of non-negative doubles), left
+// in device memory for the launches of a captured step.  out[0] = dt0, out[1] = 1 if the maximum is zero, NaN or inf
+// (the value amrhydro_cfl_dt reports as AMRHYDRO_ENONFINITE), else 0.  fixed > 0: that step size instead.
+__global__ void k_dt0(const unsigned long long *__restrict__ smax_bits, int l0, int l1, double cfl_dx0, double fixed,
+                      double *__restrict__ out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  if (fixed > 0.0) { out[0] = fixed; out[1] = 0.0; return; }
+  double s = 0.0;
+  for (int l = l0; l <= l1; ++l) {
+    const double v = __longlong_as_double((long long)smax_bits[l]);
+    if (!(v <= s)) s = v;                        // keeps NaN/inf
+  }
+  out[0] = cfl_dx0 / s;
+  out[1] = (!(s > 0.0) || !(s - s == 0.0)) ? 1.0 : 0.0;
+}
+
 // ------------------------------------------------------------------ a2: ghost fill (S5-S7)
 template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
   if (a > T(0) && b > T(0)) return tmin(a, b);
@@ -339,7 +355,8 @@ __global__ void __launch_bounds__(256) k_restrict(Pool<T> pool, int fslot, int c
 template <typename T, int NV>
 __global__ void __launch_bounds__(64) k_flux_registers(int first, int level, const Desc *__restrict__ desc,
                                                        const int *__restrict__ child, const T *__restrict__ bflux,
-                                                       T *__restrict__ Rf, T *__restrict__ Rc, T wdt) {
+                                                       T *__restrict__ Rf, T *__restrict__ Rc, T wdt, double w, DtDev dtd) {
+  if (dtd.p) wdt = T(w * (*dtd.p * dtd.pow2));
   const int pl = blockIdx.x, p = first + pl, task = blockIdx.y;
   const int ca = threadIdx.x & 7, cb = threadIdx.x >> 3;
   if (task < 6) {

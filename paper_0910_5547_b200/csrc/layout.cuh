@@ -48,6 +48,15 @@ struct Desc {
   int nbr[27];
 };
 
+// Time step of a launch when it lives in device memory (CUDA-graph replay of the subcycled step: the graph's kernel
+// arguments are frozen, the step size is not): dt = dt0[0] * pow2 with pow2 = 2^-level exactly, i.e. bitwise the value the
+// host recursion dt/2 hands down.  p == nullptr: the launch carries dt as a plain argument.
+struct DtDev {
+  const double *p;
+  double pow2;
+  double hx;       // cell width of the level (rk_stage: dt/dx is formed as on the host, (dt0 * pow2) / hx)
+};
+
 template <typename T> struct Pool {
   T *base;
   int max_patches;

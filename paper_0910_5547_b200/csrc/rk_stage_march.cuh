@@ -412,8 +412,9 @@ template <typename T, int NV, bool BASE>
 __global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? (BASE && AMR_BASE_TMA ? 2 : AMR_MINB32) : 2)))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit) {
+                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd) {
   using S = mk::Smem<T, NV, false, BASE>;
+  if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
   extern __shared__ unsigned char smem_raw[];
@@ -654,7 +655,7 @@ int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int ns
 template <typename T, int NV>
 int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0) {
+                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
   static bool configured = false;
   constexpr size_t bytes0 = mk::Smem<T, NV, false, false>::BYTES, bytes1 = mk::Smem<T, NV, false, true>::BYTES;
   if (!configured) {
@@ -666,10 +667,10 @@ int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sb
   }
   if (a != T(0))
     k_rk_stage_march<T, NV, true><<<n << zsplit, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                                bflux, floor_hits, desc, direct_halo, smax_out, zsplit);
+                                                                                bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd);
   else
     k_rk_stage_march<T, NV, false><<<n << zsplit, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                                 bflux, floor_hits, desc, direct_halo, nullptr, zsplit);
+                                                                                 bflux, floor_hits, desc, direct_halo, nullptr, zsplit, dtd);
   return 0;
 }
 

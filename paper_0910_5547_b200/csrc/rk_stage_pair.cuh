@@ -39,6 +39,15 @@ template <typename T> __device__ __forceinline__ void st2(T *p, T x, T y) {
 }
 
 constexpr int THREADS = 128;
+#ifndef AMR_PK_XSHFL
+#define AMR_PK_XSHFL 1     // x exchange (q+ to the right neighbour, flux to the left one) through warp shuffles; shared memory only at the patch edge
+#endif
+
+// 64-bit shuffles inside the 8 lanes of one row (lane = (row & 3) * 8 + px)
+__device__ __forceinline__ double shfl_up8(double x) { return __shfl_up_sync(0xffffffffu, x, 1, 8); }
+__device__ __forceinline__ float shfl_up8(float x) { return __shfl_up_sync(0xffffffffu, x, 1, 8); }
+__device__ __forceinline__ double shfl_down8(double x) { return __shfl_down_sync(0xffffffffu, x, 1, 8); }
+__device__ __forceinline__ float shfl_down8(float x) { return __shfl_down_sync(0xffffffffu, x, 1, 8); }
 
 template <typename T, int NV, bool WB> struct Smem {
   static constexpr int NSLOT = 4;                  // ring of raw conserved planes (TMA)
@@ -46,7 +55,11 @@ template <typename T, int NV, bool WB> struct Smem {
   static constexpr int RAWP = NV * NI * NI;        // one raw plane [NV][16][16], dense TMA box
   static constexpr int PW = NP;                    // primitive plane [20][20]: even pitch, pairs are 16-byte aligned
   static constexpr int WV = NP * PW;
+#if AMR_PK_XSHFL
+  static constexpr int QXP = 1, QXV = 2 * NI;      // [2][16 rows]: column 0 = q+ of cell -1, column 1 = q+ of cell 15 / flux through face 16
+#else
   static constexpr int QXP = 9, QXV = NI * QXP;    // [16 rows][9]: slot t = q+ of cell 2t-1 / flux through face 2t
+#endif
   static constexpr int QYV = (NI + 1) * NI;        // [17][16]: slot j = q+ of row j-1 / flux through face j
   static constexpr int HQV = 16;                   // q- of the ghost cell 16 of every line (per direction)
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
@@ -123,7 +136,7 @@ __device__ __forceinline__ void halo_slopes(T *sm, int buf, int lane, T th2) {
   const int t = lane & 15, hi = lane >> 4;
   const T *s3 = sm + S::O_W + buf * (NV * WV) +
                 (D == 0 ? (t + NG) * PW + (hi ? NG + NI - 1 : 0) : (hi ? NG + NI - 1 : 0) * PW + (t + NG));
-  T *qlo = sm + (D == 0 ? S::O_QX + t * S::QXP : S::O_QY + t);
+  T *qlo = sm + (D == 0 ? S::O_QX + t * S::QXP : S::O_QY + t);      // (QXP = 1 with AMR_PK_XSHFL: column 0)
   T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
   constexpr int qv = D == 0 ? S::QXV : S::QYV;
 #pragma unroll
@@ -141,7 +154,7 @@ __device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T
   if (lane >= 16) return;
   const int t = lane;
   constexpr int qv = D == 0 ? S::QXV : S::QYV;
-  T *q16 = sm + (D == 0 ? S::O_QX + t * S::QXP + 8 : S::O_QY + NI * NI + t);
+  T *q16 = sm + (D == 0 ? S::O_QX + (AMR_PK_XSHFL ? NI + t : t * S::QXP + 8) : S::O_QY + NI * NI + t);
   const T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
   T WL[NV], WR[NV], G[NV];
 #pragma unroll
@@ -156,14 +169,67 @@ __device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T
   }
 }
 
+// both at once (Euler): lanes 0-15 the x faces, lanes 16-31 the y faces, with the direction a run-time value of the
+// lane.  Same operations in the same order as mk::face_flux<T, 0> / <T, 1> (B * v is written fma(B, v, 0), which rounds
+// identically), so a face shared by two patches still gets bitwise the same flux from both.
+#ifndef AMR_PK_HFLUX1
+#define AMR_PK_HFLUX1 1
+#endif
+template <typename T>
+__device__ __forceinline__ void face_flux_xy(const T (&L)[5], const T (&R)[5], const Params<T> &P, T (&G)[5], bool y) {
+  const T rl = L[0], el = L[1], rr = R[0], er = R[1];
+  const T vdl = y ? L[3] : L[2], vdr = y ? R[3] : R[2];
+  const T pl = (P.gm1 * rl) * el, pr = (P.gm1 * rr) * er;
+  const T q2l = fma(L[4], L[4], fma(L[3], L[3], L[2] * L[2]));
+  const T q2r = fma(R[4], R[4], fma(R[3], R[3], R[2] * R[2]));
+  const T hl = fma(T(0.5), q2l, el), hr = fma(T(0.5), q2r, er);
+  const T sl = tabs(vdl) + mk::fsqrt(P.gg1 * el), sr = tabs(vdr) + mk::fsqrt(P.gg1 * er);
+  const T lam = sl > sr ? sl : sr;
+  const T A = rr * (vdr - lam), B = rl * (vdl + lam);
+  const T pp = pl + pr;
+  G[0] = A + B;
+  G[1] = fma(A, R[2], fma(B, L[2], y ? T(0) : pp));
+  G[2] = fma(A, R[3], fma(B, L[3], y ? pp : T(0)));
+  G[3] = fma(A, R[4], B * L[4]);
+  G[4] = fma(A, hr, fma(B, hl, fma(pr, vdr, pl * vdl)));
+}
+template <typename T, typename S>
+__device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface) {
+  constexpr int NV = 5;
+  const int t = lane & 15, d = lane >> 4;
+  const int qv = d ? S::QYV : S::QXV;
+  T *q16 = sm + (d ? S::O_QY + NI * NI + t : S::O_QX + (AMR_PK_XSHFL ? NI + t : t * S::QXP + 8));
+  const T *hq = sm + S::O_HQ + d * (NV * S::HQV) + t;
+  T WL[NV], WR[NV], G[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) { WL[v] = q16[v * qv]; WR[v] = hq[v * S::HQV]; }
+  face_flux_xy<T>(WL, WR, P, G, d != 0);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) q16[v * qv] = G[v];
+  if (bflux) {
+    T *B = bflux + ((size_t(pl) * 9 + 3 * d + 2) * NV) * 256 + zface * 16 + t;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
+  }
+}
+
 }  // namespace pk
 
+#ifndef AMR_PK_MINB
+#define AMR_PK_MINB 2
+#endif
+#ifdef AMR_PK_MAXNREG        // tuning: an explicit register cap instead of the one implied by CTAs per SM
+#define AMR_PK_BOUNDS __maxnreg__(AMR_PK_MAXNREG)
+#else
+#define AMR_PK_BOUNDS __launch_bounds__(pk::THREADS, AMR_PK_MINB)
+#endif
 template <typename T, int NV, bool BASE>
-__global__ void __launch_bounds__(pk::THREADS, 2)
+__global__ void AMR_PK_BOUNDS
 k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                 T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit) {
+                const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd) {
   using S = pk::Smem<T, NV, BASE>;
+  if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   constexpr int PW = S::PW, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP, NSLOT = S::NSLOT;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
   extern __shared__ unsigned char smem_raw[];
@@ -237,7 +303,11 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   T *out = pool.patch(sout, p) + off;
   const T *raw = sm + S::O_RAW + j * NI + i0;                 // this pair in ring slot 0, v = 0
   T *wme = sm + S::O_W + (j + NG) * PW + (i0 + NG);           // this pair in primitive buffer 0, v = 0
+#if AMR_PK_XSHFL
+  T *qx = sm + S::O_QX + j + (px == 7 ? NI : 0);              // px = 0: q+ of cell -1 of this row; px = 7: q+ of cell 15 / flux through face 16
+#else
   T *qx = sm + S::O_QX + j * S::QXP + px;                     // slot px: q+ of cell i0-1 / flux through face i0
+#endif
   T *qy = sm + S::O_QY + j * NI + i0;                         // slot j: q+ of row j-1 / flux through face j
 
   T Uh[NV];                                                   // halo cell of the next plane to convert
@@ -315,6 +385,9 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 #pragma unroll
     for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(w + v * WV); Wc[0][v] = x.x; Wc[1][v] = x.y; }
     T qmx0[NV], qpx0[NV], qmx1[NV], qmy0[NV], qmy1[NV];
+#if AMR_PK_XSHFL
+    T WLs[NV];                                     // q+ of cell i0-1 from the left neighbour's registers (px > 0)
+#endif
     if (live) {
       // 1. slopes of both cells along x and y; publish the q+ the neighbours need
 #pragma unroll
@@ -328,7 +401,13 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         qmx0[v] = fma(-qs, mr, a0); qpx0[v] = fma(qs, mr, a0);
         mr = pk::slope_mr(d1, d2, wr - a0, th2, qs);
         qmx1[v] = fma(-qs, mr, a1);
+#if AMR_PK_XSHFL
+        const T qpx1 = fma(qs, mr, a1);
+        WLs[v] = pk::shfl_up8(qpx1);
+        if (px == 7) qx[v * QXV] = qpx1;           // for the flux through face 16 (halo_flux)
+#else
         qx[v * QXV + 1] = fma(qs, mr, a1);
+#endif
         mr = pk::slope_mr(a0 - wd.x, wu.x - a0, wu.x - wd.x, th2, qs);
         qmy0[v] = fma(-qs, mr, a0);
         const T qpy0 = fma(qs, mr, a0);
@@ -337,7 +416,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
       }
       if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
-      if (warp == ((c + 2) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
+      if (warp == ((c + (AMR_PK_HFLUX1 ? 1 : 2)) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
       arrive(0);
     }
     // 2. z (between the two halves of the barrier): slope of cell c from this pair's own planes c-1 (dzm), c, c+1;
@@ -414,7 +493,12 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       T WL[NV], WD0[NV], WD1[NV];
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
+#if AMR_PK_XSHFL
+        WL[v] = WLs[v];
+        if (px == 0) WL[v] = qx[v * QXV];          // q+ of the ghost cell -1 (halo_slopes)
+#else
         WL[v] = qx[v * QXV];
+#endif
         const auto y = pk::ld2(qy + v * QYV);
         WD0[v] = y.x; WD1[v] = y.y;
       }
@@ -423,10 +507,19 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       mk::face_flux<T, 1>(WD0, qmy0, P, Gy0);
       mk::face_flux<T, 1>(WD1, qmy1, P, Gy1);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) { qx[v * QXV] = Gx0[v]; pk::st2(qy + v * QYV, Gy0[v], Gy1[v]); }
+      for (int v = 0; v < NV; ++v) {
+#if !AMR_PK_XSHFL
+        qx[v * QXV] = Gx0[v];
+#endif
+        pk::st2(qy + v * QYV, Gy0[v], Gy1[v]);
+      }
     }
+#if AMR_PK_HFLUX1
+    if (warp == ((c + 2) & 3)) pk::halo_flux_xy<T, S>(sm, lane, P, bflux, pl, c - NG + zlo);
+#else
     if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo);
     if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo);
+#endif
     arrive(1);
     if (bflux) {
       if ((i0 & 7) == 0) {
@@ -456,7 +549,12 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
     // 5. flux differences in x and y, minus the low z face parked in acc
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
+#if AMR_PK_XSHFL
+      T fxh = pk::shfl_down8(Gx0[v]);               // flux through face i0+2 = the right neighbour's low face
+      if (px == 7) fxh = qx[v * QXV];               // face 16 (halo_flux)
+#else
       const T fxh = qx[v * QXV + 1];
+#endif
       const auto fyh = pk::ld2(qy + v * QYV + NI);
       acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) - acc[0][v];
       acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) - acc[1][v];
@@ -476,7 +574,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 template <typename T, int NV>
 int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                          T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0) {
+                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
   static bool configured = false;
 #ifndef AMR_PAIR_EXTRA_SMEM
 #define AMR_PAIR_EXTRA_SMEM 0     // experiment: pad the allocation to force one CTA per SM
@@ -491,10 +589,10 @@ int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sba
   }
   if (a != T(0))
     k_rk_stage_pair<T, NV, true><<<n << zsplit, pk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                              bflux, floor_hits, desc, direct_halo, smax_out, zsplit);
+                                                                              bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd);
   else
     k_rk_stage_pair<T, NV, false><<<n << zsplit, pk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                               bflux, floor_hits, desc, direct_halo, nullptr, zsplit);
+                                                                               bflux, floor_hits, desc, direct_halo, nullptr, zsplit, dtd);
   return 0;
 }
 

@@ -43,7 +43,8 @@ __device__ __forceinline__ void ref_direction(const T *__restrict__ Uin, int c, 
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_rk_stage_ref(Pool<T> pool, int sin, int sbase, int sout, int first,
                                                       T a, T b, T dtdx, Params<T> P, T *__restrict__ bflux,
-                                                      unsigned long long *__restrict__ floor_hits) {
+                                                      unsigned long long *__restrict__ floor_hits, DtDev dtd) {
+  if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   const int pl = blockIdx.x, p = first + pl;
   const int i = threadIdx.x & 15, j = threadIdx.x >> 4, k = blockIdx.y;
   const T *Uin = pool.patch(sin, p);
