@@ -43,6 +43,11 @@ struct amrhydro {
   Desc *d_desc = nullptr;
   int *d_child = nullptr, *d_octant = nullptr;
   void *d_Rf = nullptr, *d_Rc = nullptr, *d_bflux = nullptr;
+  // found once per hierarchy, so that the per-level launches carry no idle blocks: patches with a coarse-fine region
+  // (k_fill_ghosts when sibling copies are skipped), flux-register tasks (local patch * 64 + task of k_flux_registers),
+  // and per patch the boundary-flux planes a register reads (bit 3 d + s; rk_stage stores only those)
+  int *d_cflist = nullptr, *d_frtasks = nullptr, *d_bneed = nullptr;
+  std::vector<int> cf_first, cf_count, fr_first, fr_count;
   size_t bflux_patches = 0;
   unsigned long long *d_scalars = nullptr;  // [0] scratch, [1] floor hits
   unsigned long long *d_smax = nullptr;     // per level: bits of the max signal speed of (level, smax_slot[level])
@@ -156,6 +161,8 @@ void free_hierarchy(amrhydro *h) {
   drop_graph(h);
   cudaFree(h->d_desc); cudaFree(h->d_child); cudaFree(h->d_octant);
   cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux); cudaFree(h->d_smax);
+  cudaFree(h->d_cflist); cudaFree(h->d_frtasks); cudaFree(h->d_bneed);
+  h->d_cflist = h->d_frtasks = h->d_bneed = nullptr;
   h->d_smax = nullptr;
   h->smax_slot.clear();
   h->d_desc = nullptr; h->d_child = h->d_octant = nullptr;
@@ -390,6 +397,43 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
   CUDA_TRY(h, cudaMemcpyAsync(h->d_desc, h->tbl.data(), size_t(np) * sizeof(Desc), cudaMemcpyHostToDevice, h->stream));
   CUDA_TRY(h, cudaMemcpyAsync(h->d_child, h->child.data(), size_t(np) * 8 * sizeof(int), cudaMemcpyHostToDevice, h->stream));
   CUDA_TRY(h, cudaMemcpyAsync(h->d_octant, h->octant.data(), size_t(np) * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+  {
+    std::vector<int> cfl, frt, bneed(np, 0);
+    h->cf_first.assign(nlev, 0); h->cf_count.assign(nlev, 0); h->fr_first.assign(nlev, 0); h->fr_count.assign(nlev, 0);
+    for (int l = 0; l < nlev; ++l) {
+      h->cf_first[l] = int(cfl.size());
+      h->fr_first[l] = int(frt.size());
+      for (int p = first[l]; p < first[l] + count[l]; ++p) {
+        bool cf = false;
+        for (int r = 0; r < 27; ++r) cf |= (r != 13 && tbl[p].nbr[r] == -1);
+        if (cf) cfl.push_back(p);
+        const int pl = p - first[l];
+        for (int f = 0; f < 6; ++f)                           // fine side of a coarse-fine face
+          if (l > 0 && tbl[p].nbr[face_region(f)] == -1) {
+            frt.push_back(pl * 64 + f);
+            bneed[p] |= 1 << ((f >> 1) * 3 + ((f & 1) ? 2 : 0));
+          }
+        for (int o = 0; o < 8; ++o) {                         // coarse side: the face of a child that has no sibling there
+          const int ch = child[size_t(p) * 8 + o];
+          if (ch < 0) continue;
+          for (int f = 0; f < 6; ++f)
+            if (tbl[ch].nbr[face_region(f)] == -1) {
+              frt.push_back(pl * 64 + 6 + o * 6 + f);
+              bneed[p] |= 1 << ((f >> 1) * 3 + ((o >> (f >> 1)) & 1) + (f & 1));
+            }
+        }
+      }
+      h->cf_count[l] = int(cfl.size()) - h->cf_first[l];
+      h->fr_count[l] = int(frt.size()) - h->fr_first[l];
+    }
+    CUDA_TRY(h, cudaMalloc(&h->d_cflist, std::max<size_t>(1, cfl.size()) * sizeof(int)));
+    CUDA_TRY(h, cudaMalloc(&h->d_frtasks, std::max<size_t>(1, frt.size()) * sizeof(int)));
+    CUDA_TRY(h, cudaMalloc(&h->d_bneed, size_t(np) * sizeof(int)));
+    // (synchronous copies from these locals; the stream is idle: synchronised above)
+    if (!cfl.empty()) CUDA_TRY(h, cudaMemcpy(h->d_cflist, cfl.data(), cfl.size() * sizeof(int), cudaMemcpyHostToDevice));
+    if (!frt.empty()) CUDA_TRY(h, cudaMemcpy(h->d_frtasks, frt.data(), frt.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CUDA_TRY(h, cudaMemcpy(h->d_bneed, bneed.data(), size_t(np) * sizeof(int), cudaMemcpyHostToDevice));
+  }
   if (nlev > 1) {
     size_t rb = size_t(np) * 6 * h->nv * 64 * elem(h);
     CUDA_TRY(h, cudaMalloc(&h->d_Rf, rb));
@@ -556,8 +600,11 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
     if (phase1) {
-      k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
-          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, skip);
+      // sibling copies skipped: only the patches with a coarse-fine region have anything to fill
+      const int nb = skip ? h->cf_count[level] : h->lev_count[level];
+      k_fill_ghosts<T, NV><<<dim3(nb, NP), 256, 0, h->stream>>>(
+          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, skip,
+          skip ? h->d_cflist + h->cf_first[level] : nullptr);
       LAUNCH_CHECK(h);
     }
     if (phase2) {
@@ -577,7 +624,7 @@ static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
     k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
-        make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2);
+        make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2, nullptr);
     LAUNCH_CHECK(h);
     return 0;
   });
@@ -610,7 +657,7 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       if constexpr (NV == 5) {
         int r = launch_rk_stage_pair<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                             make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                            fuse ? h->d_smax + level : nullptr, zs, dtd);
+                                            fuse ? h->d_smax + level : nullptr, zs, dtd, h->d_bneed);
         if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_pair: ") + cudaGetErrorString((cudaError_t)r));
         LAUNCH_CHECK(h);
       }
@@ -622,9 +669,10 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       LAUNCH_CHECK(h);
     }
     if (fuse) h->smax_slot[level] = sout;
-    if (regs) {
-      k_flux_registers<T, NV><<<dim3(n, 54), 64, 0, h->stream>>>(first, level, h->d_desc, h->d_child, bflux,
-                                                                  (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt), w, dtd);
+    if (regs && h->fr_count[level] > 0) {
+      k_flux_registers<T, NV><<<h->fr_count[level], 64, 0, h->stream>>>(first, level, h->d_desc, h->d_child, bflux,
+                                                                         (T *)h->d_Rf, (T *)h->d_Rc, T(w * dt), w, dtd,
+                                                                         h->d_frtasks + h->fr_first[level]);
       LAUNCH_CHECK(h);
     }
     return 0;

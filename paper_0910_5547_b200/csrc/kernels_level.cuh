@@ -127,14 +127,17 @@ template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
                                                      int first, const Desc *__restrict__ desc,
-                                                     const int *__restrict__ octant, int mode) {
+                                                     const int *__restrict__ octant, int mode,
+                                                     const int *__restrict__ plist) {
   // Latency is what this kernel costs on small AMR levels, so it is written as two dependent round trips to
   // memory: (1) the patch's descriptor row and octant (every thread reads what it needs, broadcast through
   // L1: no staging, no barrier), (2) all parent cells this plane prolongates from -- 3 coarse planes x 12 x 12
   // per variable, time-interpolated once (S7) into shared memory -- together with the sibling cells to copy.
   // A fine patch is an octant of its parent and origins are multiples of 16, so parent indices follow from
   // the octant bits alone: coarse index of padded fine index t along d = 8 oc_d + floor((t - 2) / 2) + 2.
-  const int p = first + blockIdx.x, k = blockIdx.y;
+  // plist (may be null): the patches of the level that have a coarse-fine region (all this launch has to fill when
+  // the sibling copies are skipped), so that a level of thousands of interior patches launches no idle blocks
+  const int p = plist ? plist[blockIdx.x] : first + blockIdx.x, k = blockIdx.y;
   const Desc &D = desc[p];
   T *U = pool.patch(slot, p);
   constexpr int CT = 12, CTV = 3 * CT * CT;
@@ -355,9 +358,12 @@ __global__ void __launch_bounds__(256) k_restrict(Pool<T> pool, int fslot, int c
 template <typename T, int NV>
 __global__ void __launch_bounds__(64) k_flux_registers(int first, int level, const Desc *__restrict__ desc,
                                                        const int *__restrict__ child, const T *__restrict__ bflux,
-                                                       T *__restrict__ Rf, T *__restrict__ Rc, T wdt, double w, DtDev dtd) {
+                                                       T *__restrict__ Rf, T *__restrict__ Rc, T wdt, double w, DtDev dtd,
+                                                       const int *__restrict__ tasks) {
   if (dtd.p) wdt = T(w * (*dtd.p * dtd.pow2));
-  const int pl = blockIdx.x, p = first + pl, task = blockIdx.y;
+  // tasks (may be null): the (patch, face) and (patch, octant, face) pairs of the level that lie on a coarse-fine
+  // boundary, packed as local patch * 64 + task, found once per hierarchy; null: every block tests its own pair
+  const int pl = tasks ? tasks[blockIdx.x] >> 6 : blockIdx.x, p = first + pl, task = tasks ? tasks[blockIdx.x] & 63 : blockIdx.y;
   const int ca = threadIdx.x & 7, cb = threadIdx.x >> 3;
   if (task < 6) {
     const int f = task;

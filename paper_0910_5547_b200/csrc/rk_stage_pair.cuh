@@ -194,7 +194,8 @@ __device__ __forceinline__ void face_flux_xy(const T (&L)[5], const T (&R)[5], c
   G[4] = fma(A, hr, fma(B, hl, fma(pr, vdr, pl * vdl)));
 }
 template <typename T, typename S>
-__device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface) {
+__device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface,
+                                             int bmask) {
   constexpr int NV = 5;
   const int t = lane & 15, d = lane >> 4;
   const int qv = d ? S::QYV : S::QXV;
@@ -206,7 +207,7 @@ __device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P
   face_flux_xy<T>(WL, WR, P, G, d != 0);
 #pragma unroll
   for (int v = 0; v < NV; ++v) q16[v * qv] = G[v];
-  if (bflux) {
+  if (bflux && ((bmask >> (3 * d + 2)) & 1)) {
     T *B = bflux + ((size_t(pl) * 9 + 3 * d + 2) * NV) * 256 + zface * 16 + t;
 #pragma unroll
     for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
@@ -227,7 +228,8 @@ template <typename T, int NV, bool BASE>
 __global__ void AMR_PK_BOUNDS
 k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                 T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd) {
+                const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd,
+                const int *__restrict__ bneed) {
   using S = pk::Smem<T, NV, BASE>;
   if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   constexpr int PW = S::PW, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP, NSLOT = S::NSLOT;
@@ -247,6 +249,8 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
   const T th2 = T(2) * P.theta;
   int hits = 0;
+  // which of the nine boundary-flux planes of this patch a flux register will read (bit 3 d + s; all when no table)
+  const int bmask = bflux ? (bneed ? bneed[p] : 0x1ff) : 0;
 
   if (tid == 0) {
 #pragma unroll
@@ -446,7 +450,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         mk::face_flux<T, 2>(L0, qm[0], P, Gz[0]);
         mk::face_flux<T, 2>(L1, qm[1], P, Gz[1]);
       }
-      if (bflux && ((c - NG + zlo) & 7) == 0) {
+      if (((c - NG + zlo) & 7) == 0 && ((bmask >> (6 + ((c - NG + zlo) >> 3))) & 1)) {
         T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG + zlo) >> 3)) * NV) * 256 + j * 16 + i0;
 #pragma unroll
         for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gz[0][v], T(0.5) * Gz[1][v]);
@@ -515,19 +519,19 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       }
     }
 #if AMR_PK_HFLUX1
-    if (warp == ((c + 2) & 3)) pk::halo_flux_xy<T, S>(sm, lane, P, bflux, pl, c - NG + zlo);
+    if (warp == ((c + 2) & 3)) pk::halo_flux_xy<T, S>(sm, lane, P, bflux, pl, c - NG + zlo, bmask);
 #else
     if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo);
     if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo);
 #endif
     arrive(1);
-    if (bflux) {
-      if ((i0 & 7) == 0) {
+    if (bmask) {
+      if ((i0 & 7) == 0 && ((bmask >> (i0 >> 3)) & 1)) {
         T *B = bflux + ((size_t(pl) * 9 + 0 + (i0 >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + j;
 #pragma unroll
         for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * Gx0[v];
       }
-      if ((j & 7) == 0) {
+      if ((j & 7) == 0 && ((bmask >> (3 + (j >> 3))) & 1)) {
         T *B = bflux + ((size_t(pl) * 9 + 3 + (j >> 3)) * NV) * 256 + (c - NG + zlo) * 16 + i0;
 #pragma unroll
         for (int v = 0; v < NV; ++v) pk::st2(B + v * 256, T(0.5) * Gy0[v], T(0.5) * Gy1[v]);
@@ -574,7 +578,8 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 template <typename T, int NV>
 int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                          T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
+                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0},
+                         const int *bneed = nullptr) {
   static bool configured = false;
 #ifndef AMR_PAIR_EXTRA_SMEM
 #define AMR_PAIR_EXTRA_SMEM 0     // experiment: pad the allocation to force one CTA per SM
@@ -589,10 +594,10 @@ int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sba
   }
   if (a != T(0))
     k_rk_stage_pair<T, NV, true><<<n << zsplit, pk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                              bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd);
+                                                                              bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd, bneed);
   else
     k_rk_stage_pair<T, NV, false><<<n << zsplit, pk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                               bflux, floor_hits, desc, direct_halo, nullptr, zsplit, dtd);
+                                                                               bflux, floor_hits, desc, direct_halo, nullptr, zsplit, dtd, bneed);
   return 0;
 }
 
