@@ -177,6 +177,18 @@ int amrhydro_copy_slot(amrhydro_t *h, int level, int src_slot, int dst_slot);
  * parent in `parent_slot` (conservative limited-linear, the operator of S6); the parent's ghosts must be
  * filled.  AMRHYDRO_EINVAL for a level-0 patch. */
 int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_octmax);
+/* regrid (NEXT-3): a new descriptor table on the bound, live pool, with no host round trip of cell data.
+ * new_tbl / np_new / nlev_new: as for amrhydro_set_hierarchy (same validation; dx0 and bc are kept);
+ * old_of_new[np_new] (host): index of the same patch (same level and origin) in the current table, or -1 for a
+ * patch that did not exist.  `slot` holds the state before and after; every other slot is scratch afterwards
+ * (needs nslots >= 2 and np_new <= max_patches).  In order: (1) amrhydro_restrict of every fine level into
+ * `slot`, so that the cells under a removed fine patch hold its average (S8); (2) surviving patches are moved to
+ * their new index by a device kernel (k_move_patches, through the scratch slot); (3) the table, flux registers and
+ * launch lists are rebuilt; (4) from level 0 up, ghosts are filled and the new patches of the next level are
+ * prolongated from their parents (S21), one launch per level.  Synchronises.  On AMRHYDRO_EINVAL the old hierarchy
+ * and `slot` are unchanged. */
+int amrhydro_regrid(amrhydro_t *h, const amrhydro_patch_desc *new_tbl, int np_new, int nlev_new,
+                    const int *old_of_new, int slot);
 int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slot);
 
 /* nvars = 9 only (AMRHYDRO_EINVAL otherwise): psi <- factor * psi on the interior cells of one level,

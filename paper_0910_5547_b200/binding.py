@@ -22,7 +22,7 @@ EXPORTS = [
     "amrhydro_upload", "amrhydro_download", "amrhydro_download_padded", "amrhydro_download_registers",
     "amrhydro_cfl_dt", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
     "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_refine_indicator",
-    "amrhydro_prolong_interior", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
+    "amrhydro_prolong_interior", "amrhydro_regrid", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
 ]
 
 
@@ -68,6 +68,7 @@ def load_library():
     L.amrhydro_glm_damp.argtypes = [vp, i, i, d]
     L.amrhydro_refine_indicator.argtypes = [vp, i, i, dp]
     L.amrhydro_prolong_interior.argtypes = [vp, i, i, i]
+    L.amrhydro_regrid.argtypes = [vp, C.POINTER(PatchDesc), i, i, C.POINTER(C.c_int), i]
     L.amrhydro_advance.argtypes = [vp, d, d, dp]
     L.amrhydro_advance_host.argtypes = [vp, d, d, i, vp, vp, dp]
     L.amrhydro_sync.argtypes = [vp]
@@ -83,7 +84,7 @@ class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
     def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=3, halo=1,
-                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2, graph=0):
+                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2, graph=0, max_patches=None):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():
             raise AmrHydroError("no CUDA device: the amrhydro path has no CPU fallback")
@@ -105,20 +106,36 @@ class AmrHydro:
         self.npatch = int(hier["level"].shape[0])
         nlev = int(hier["nlevels"])
         self.nslots = nslots or (3 if nlev > 1 else 2)
-        nbytes = self.L.amrhydro_pool_bytes(self.h, self.npatch, self.nslots)
+        self.max_patches = max(self.npatch, int(max_patches or 0))     # room for a later regrid
+        nbytes = self.L.amrhydro_pool_bytes(self.h, self.max_patches, self.nslots)
         self.pool = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self._ok(self.L.amrhydro_bind_pool(self.h, self.pool.data_ptr(), nbytes, self.npatch, self.nslots,
+        self._ok(self.L.amrhydro_bind_pool(self.h, self.pool.data_ptr(), nbytes, self.max_patches, self.nslots,
                                            self.stream.cuda_stream))
-        tbl = (PatchDesc * self.npatch)()
+        tbl = self._table(hier)
+        bc = (C.c_int * 6)(*[int(x) for x in hier["bc"]])
+        self._ok(self.L.amrhydro_set_hierarchy(self.h, tbl, self.npatch, nlev, float(hier["dx0"]), bc))
+
+    @staticmethod
+    def _table(hier):
+        n = int(hier["level"].shape[0])
+        tbl = (PatchDesc * n)()
         lv, org, par, nbr = (np.ascontiguousarray(hier[k], dtype=np.int32) for k in ("level", "origin", "parent", "nbr"))
-        view = np.frombuffer(tbl, dtype=np.int32).reshape(self.npatch, 32)
+        view = np.frombuffer(tbl, dtype=np.int32).reshape(n, 32)
         view[:, 0] = lv
         view[:, 1:4] = org
         view[:, 4] = par
         view[:, 5:32] = nbr
-        bc = (C.c_int * 6)(*[int(x) for x in hier["bc"]])
-        self._ok(self.L.amrhydro_set_hierarchy(self.h, tbl, self.npatch, nlev, float(hier["dx0"]), bc))
+        return tbl
+
+    def regrid(self, hier, old_of_new, slot=0):
+        """amrhydro_regrid: the new table on the live pool (needs max_patches >= the new patch count)."""
+        n = int(hier["level"].shape[0])
+        m = np.ascontiguousarray(old_of_new, dtype=np.int32)
+        assert m.shape == (n,)
+        self._ok(self.L.amrhydro_regrid(self.h, self._table(hier), n, int(hier["nlevels"]),
+                                        m.ctypes.data_as(C.POINTER(C.c_int)), slot))
+        self.hier, self.npatch = hier, n
 
     def _ok(self, r):
         if r != 0:

@@ -313,11 +313,9 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   return 0;
 }
 
-int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
-  if (int r = check_ready(h, false)) return r;
-  if (!tbl || !bc || np <= 0 || nlev <= 0 || !(dx0 > 0)) return fail(h, AMRHYDRO_EINVAL, "bad hierarchy arguments");
-  if (np > h->maxp) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
-  std::vector<int> first(nlev, -1), count(nlev, 0), child(size_t(np) * 8, -1), octant(np, 0);
+// everything amrhydro_set_hierarchy checks about a table, without touching the handle's state
+static int check_table(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, const int *bc, std::vector<int> &first,
+                       std::vector<int> &count, std::vector<int> &child, std::vector<int> &octant) {
   for (int p = 0; p < np; ++p) {
     const auto &d = tbl[p];
     if (d.level < 0 || d.level >= nlev) return fail(h, AMRHYDRO_EINVAL, "patch level out of range");
@@ -374,6 +372,15 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
           return fail(h, AMRHYDRO_EINVAL, "physical-boundary face entries must match the faces on the domain boundary");
       }
   }
+  return 0;
+}
+
+int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
+  if (int r = check_ready(h, false)) return r;
+  if (!tbl || !bc || np <= 0 || nlev <= 0 || !(dx0 > 0)) return fail(h, AMRHYDRO_EINVAL, "bad hierarchy arguments");
+  if (np > h->maxp) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
+  std::vector<int> first(nlev, -1), count(nlev, 0), child(size_t(np) * 8, -1), octant(np, 0);
+  if (int r = check_table(h, tbl, np, nlev, bc, first, count, child, octant)) return r;
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   free_hierarchy(h);
   h->tbl.assign(tbl, tbl + np);
@@ -760,10 +767,105 @@ int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slo
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    k_prolong_interior<T, NV><<<NI, 256, 0, h->stream>>>(make_pool<T>(h), slot, parent_slot, patch, h->d_desc);
+    k_prolong_interior<T, NV><<<NI, 256, 0, h->stream>>>(make_pool<T>(h), slot, parent_slot, patch, h->d_desc, nullptr);
     LAUNCH_CHECK(h);
     return 0;
   });
+}
+
+int amrhydro_regrid(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np_new, int nlev_new, const int *old_of_new, int slot) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (!tbl || !old_of_new || np_new <= 0 || nlev_new <= 0) return fail(h, AMRHYDRO_EINVAL, "bad regrid arguments");
+  if (h->nslots < 2) return fail(h, AMRHYDRO_ESTATE, "regrid needs a second slot as scratch");
+  if (np_new > h->maxp) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
+  {
+    std::vector<char> used(h->np, 0);
+    for (int q = 0; q < np_new; ++q) {
+      const int o = old_of_new[q];
+      if (o < -1 || o >= h->np) return fail(h, AMRHYDRO_EINVAL, "old_of_new out of range");
+      if (o < 0) {
+        if (tbl[q].level == 0) return fail(h, AMRHYDRO_EINVAL, "a new patch needs a parent to be prolongated from");
+        continue;
+      }
+      if (used[o]) return fail(h, AMRHYDRO_EINVAL, "old_of_new names a patch twice");
+      used[o] = 1;
+      const auto &a = h->tbl[o];
+      if (a.level != tbl[q].level || a.origin[0] != tbl[q].origin[0] || a.origin[1] != tbl[q].origin[1] ||
+          a.origin[2] != tbl[q].origin[2])
+        return fail(h, AMRHYDRO_EINVAL, "a surviving patch must keep its level and origin");
+    }
+  }
+  {
+    std::vector<int> first(nlev_new, -1), count(nlev_new, 0), child(size_t(np_new) * 8, -1), octant(np_new, 0);
+    if (int r = check_table(h, tbl, np_new, nlev_new, h->bc, first, count, child, octant)) return r;
+  }
+  const int scratch = (slot + 1) % h->nslots;
+  // (1) the cells under fine patches hold the fine average before any fine patch disappears (S8)
+  for (int l = h->nlev - 1; l >= 1; --l)
+    if (int r = amrhydro_restrict(h, l, slot, slot)) return r;
+  // (2) survivors to their new index, through the scratch slot
+  int *d_map = nullptr;
+  CUDA_TRY(h, cudaMalloc(&d_map, size_t(np_new) * sizeof(int)));
+  cudaError_t e = cudaMemcpyAsync(d_map, old_of_new, size_t(np_new) * sizeof(int), cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) {
+    dispatch(h, [&](auto t, auto nv) {
+      using T = decltype(t);
+      k_move_patches<T><<<np_new, 256, 0, h->stream>>>(make_pool<T>(h), slot, scratch, d_map);
+      (void)nv;
+      return 0;
+    });
+    ++h->launches;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) { cudaFree(d_map); return fail(h, AMRHYDRO_ECUDA, std::string("regrid move: ") + cudaGetErrorString(e)); }
+  // (3) the new table (validated like any other; on failure the old hierarchy is still in place and `slot` untouched)
+  const double dx0 = h->dx0;
+  int bc[6];
+  for (int i = 0; i < 6; ++i) bc[i] = h->bc[i];
+  if (int r = amrhydro_set_hierarchy(h, tbl, np_new, nlev_new, dx0, bc)) { cudaFree(d_map); return r; }
+  {
+    const size_t per = size_t(h->nv) * vs(h) * elem(h);
+    char *base = (char *)h->pool;
+    e = cudaMemcpyAsync(base + size_t(slot) * h->maxp * per, base + size_t(scratch) * h->maxp * per, size_t(np_new) * per,
+                        cudaMemcpyDeviceToDevice, h->stream);
+    if (e != cudaSuccess) { cudaFree(d_map); return fail(h, AMRHYDRO_ECUDA, std::string("regrid copy: ") + cudaGetErrorString(e)); }
+  }
+  // (4) level by level: ghosts of level l, then the new patches of level l + 1 from their parents (S21), one launch
+  std::vector<int> newp;
+  std::vector<int> nfirst(nlev_new + 1, 0);
+  for (int l = 1; l < nlev_new; ++l) {
+    nfirst[l] = int(newp.size());
+    for (int q = h->lev_first[l]; q < h->lev_first[l] + h->lev_count[l]; ++q)
+      if (old_of_new[q] < 0) newp.push_back(q);
+  }
+  nfirst[nlev_new] = int(newp.size());
+  int rc = 0;
+  if (!newp.empty()) {
+    e = cudaMemcpyAsync(d_map, newp.data(), newp.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) rc = fail(h, AMRHYDRO_ECUDA, std::string("regrid list: ") + cudaGetErrorString(e));
+    int last = 0;                             // the coarsest-to-finest chain of ghost fills ends below the last new patch
+    for (int l = 1; l < nlev_new; ++l)
+      if (nfirst[l + 1] > nfirst[l]) last = l;
+    for (int l = 0; l < last && !rc; ++l) {
+      const int cnt = nfirst[l + 2] - nfirst[l + 1];
+      if ((rc = amrhydro_fill_ghosts(h, l, slot, slot, slot, 0.0))) break;
+      if (cnt <= 0) continue;
+      smax_touch(h, l + 1, slot);
+      rc = dispatch(h, [&](auto t, auto nv) {
+        using T = decltype(t);
+        constexpr int NV = decltype(nv)::value;
+        k_prolong_interior<T, NV><<<dim3(NI, cnt), 256, 0, h->stream>>>(make_pool<T>(h), slot, slot, 0, h->d_desc,
+                                                                        d_map + nfirst[l + 1]);
+        LAUNCH_CHECK(h);
+        return 0;
+      });
+    }
+  }
+  cudaStreamSynchronize(h->stream);          // newp / d_map outlive the asynchronous copies
+  cudaFree(d_map);
+  return rc;
 }
 
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {

@@ -294,7 +294,8 @@ __global__ void __launch_bounds__(256) k_refine_indicator(Pool<T> pool, int slot
 // S21: all interior cells of fine patch p from its parent's padded box (operator of S6, one slot).
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_prolong_interior(Pool<T> pool, int slot, int pslot, int p,
-                                                          const Desc *__restrict__ desc) {
+                                                          const Desc *__restrict__ desc, const int *__restrict__ plist) {
+  if (plist) p = plist[blockIdx.y];                              // batched: one grid row of 16 blocks per listed patch
   const Desc &D = desc[p];
   const int Q = D.parent;
   T *U = pool.patch(slot, p);
@@ -326,6 +327,19 @@ __global__ void __launch_bounds__(256) k_prolong_interior(Pool<T> pool, int slot
     for (int d = 0; d < 3; ++d) val = val + sg[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
     U[size_t(v) * Layout<T>::VS + me] = val;
   }
+}
+
+// Regrid (NEXT-3): surviving patches move to their index in the new table.  One block per new patch; map[q] = index
+// in the old table or -1 (new patch: left for k_prolong_interior).  Whole padded boxes, 16-byte copies, from one
+// slot to another (never in place).
+template <typename T>
+__global__ void __launch_bounds__(256) k_move_patches(Pool<T> pool, int src_slot, int dst_slot, const int *__restrict__ map) {
+  const int q = blockIdx.x, o = map[q];
+  if (o < 0) return;
+  const uint4 *s = reinterpret_cast<const uint4 *>(pool.patch(src_slot, o));
+  uint4 *d = reinterpret_cast<uint4 *>(pool.patch(dst_slot, q));
+  const int n = int(size_t(pool.nv) * Layout<T>::VS * sizeof(T) / sizeof(uint4));
+  for (int c = threadIdx.x; c < n; c += 256) d[c] = s[c];
 }
 
 // ------------------------------------------------------------------ a7: restriction (S8)

@@ -146,3 +146,126 @@ def test_one_regrid_cycle_host_driven(gpu):
         g.advance(0.3, dt)
     G, O = g.download(0), o.download(0)
     assert np.isfinite(G).all() and norm_err(G, O).max() <= 1e-12
+
+
+# ------------------------------------------------------------------ amrhydro_regrid: the cycle on the live pool
+def old_of_new(h_old, h_new):
+    """Index in the old table of every patch of the new one (same level and origin), -1 for a new patch."""
+    key = {(int(l), tuple(int(c) for c in o)): p for p, (l, o) in enumerate(zip(h_old["level"], h_old["origin"]))}
+    return np.array([key.get((int(l), tuple(int(c) for c in o)), -1) for l, o in zip(h_new["level"], h_new["origin"])], np.int32)
+
+
+def oracle_regrid(o_old, h_old, h_new, gamma, nv):
+    """The same cycle with the oracle's primitives and a host copy: restrict, carry the survivors over, fill ghosts level
+    by level, prolongate the new patches (S8, S21)."""
+    import oracle
+    for l in range(h_old["nlevels"] - 1, 0, -1):
+        o_old.restrict(l)
+    Uo = o_old.download(0)
+    m = old_of_new(h_old, h_new)
+    U = np.zeros((len(m), nv, 16, 16, 16))
+    U[m >= 0] = Uo[m[m >= 0]]
+    o = oracle.Oracle(h_new, gamma, nv, threads=8)
+    o.upload(0, U)
+    for l in range(h_new["nlevels"] - 1):
+        o.fill_ghosts(l, 0, 0, 0, 0.0)
+        for p in wl.level_patches(h_new, l + 1):
+            if m[p] < 0:
+                o.prolong_interior(int(p))
+    return o, m
+
+
+def test_regrid_one_level_to_two_on_the_live_pool(gpu):
+    """test_one_regrid_cycle_host_driven with the new handle and the re-upload replaced by amrhydro_regrid."""
+    import oracle
+    nb = 3
+    h0 = wl.uniform_hierarchy(nb, periodic=True)
+    U0 = blob_state(h0, seed=5, noise=1e-3)
+    g = gpu.AmrHydro(h0, 1.4, 5, halo=1, nslots=3, max_patches=400)
+    o0 = oracle.Oracle(h0, 1.4, 5, threads=8)
+    g.upload(0, U0); o0.upload(0, U0)
+    g.fill_ghosts(0, 0)
+    ind = g.refine_indicator(0)
+    flags = ind > 0.1 * ind.max()
+    org = np.asarray(h0["origin"]) // 16
+    marked = np.zeros((2 * nb,) * 3, bool)
+    for p in range(len(org)):
+        for oc in range(8):
+            if flags[p, oc]:
+                marked[2 * org[p][0] + (oc & 1), 2 * org[p][1] + ((oc >> 1) & 1), 2 * org[p][2] + (oc >> 2)] = True
+    fine = [tuple(int(c) for c in b) for b in np.argwhere(marked)]
+    h1 = wl.build_hierarchy((nb,) * 3, [fine], (0,) * 6)
+    o, m = oracle_regrid(o0, h0, h1, 1.4, 5)
+    assert (m >= 0).sum() == len(h0["level"]) and (m < 0).sum() == len(fine)
+    launches = g.get_counter(gpu.CNT_LAUNCHES, reset=True)
+    g.regrid(h1, m)
+    assert g.get_counter(gpu.CNT_LAUNCHES) <= 4            # move, ghost fill of level 0, ONE prolongation launch for all new patches
+    G, O = g.download(0), o.download(0)
+    assert norm_err(G, O).max() <= 4e-16
+    for _ in range(2):
+        dt = o.advance(0.3)
+        assert abs(g.advance(0.3) - dt) <= 1e-12 * dt
+    G, O = g.download(0), o.download(0)
+    assert np.isfinite(G).all() and norm_err(G, O).max() <= 1e-12
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_regrid_moves_keeps_removes_and_creates(gpu, dtype):
+    """Three levels -> three levels with other blocks: some patches survive at another index, some disappear (their
+    parents keep the restricted data), some are new on levels 1 and 2 (a new level-2 patch under a new level-1 patch
+    included).  One step before, two after, oracle alongside."""
+    import oracle
+    nb = 2
+    A1 = [(i, j, k) for i in (1, 2) for j in (1, 2) for k in (1, 2)]
+    A2 = [(i, j, k) for i in (3, 4) for j in (3, 4) for k in (3, 4)]
+    B1 = [(i, j, k) for i in (1, 2, 3) for j in (1, 2) for k in (1, 2)]            # grown along x
+    B2 = [(i, j, k) for i in (4, 5, 6) for j in (3, 4) for k in (3, 4)]            # shifted along x: (3,..) removed, (5,..),(6,..) new
+    hA = wl.build_hierarchy((nb,) * 3, [A1, A2], (0,) * 6)
+    hB = wl.build_hierarchy((nb,) * 3, [B1, B2], (0,) * 6)
+    U = blob_state(hA, seed=11, w=0.25)
+    if dtype == "f32":
+        U = U.astype(np.float32).astype(np.float64)
+    g = gpu.AmrHydro(hA, 1.4, 5, dtype=dtype, max_patches=len(hB["level"]) + 8)
+    oA = oracle.Oracle(hA, 1.4, 5, threads=8)
+    g.upload(0, U); oA.upload(0, U)
+    for x in (g, oA):
+        x.restrict(2); x.restrict(1)
+    dt = oA.advance(0.3)
+    g.advance(0.3, dt)
+    oB, m = oracle_regrid(oA, hA, hB, 1.4, 5)
+    moved = [(int(a), q) for q, a in enumerate(m) if a >= 0 and a != q]
+    assert moved and (m < 0).sum() >= 8 and len(set(range(len(hA["level"]))) - set(m.tolist())) >= 4
+    g.regrid(hB, m)
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    # (the state carries the round-off of the step before the regrid: rho v_y is ~0 in this blob, its norm is tiny)
+    assert norm_err(g.download(0).astype(np.float64), oB.download(0), vector=(dtype == "f32")).max() <= tol
+    for _ in range(2):
+        dt = oB.advance(0.3)
+        g.advance(0.3, dt)
+    G, O = g.download(0).astype(np.float64), oB.download(0)
+    assert np.isfinite(G).all() and norm_err(G, O, vector=(dtype == "f32")).max() <= tol
+
+
+def test_regrid_rejects_bad_maps(gpu):
+    h0 = wl.uniform_hierarchy(2, periodic=True)
+    fine = [(i, j, k) for i in (1, 2) for j in (1, 2) for k in (1, 2)]
+    h1 = wl.build_hierarchy((2, 2, 2), [fine], (0,) * 6)
+    g = gpu.AmrHydro(h0, 1.4, 5, nslots=3, max_patches=32)
+    U0 = blob_state(h0, seed=2)
+    g.upload(0, U0)
+    m = old_of_new(h0, h1)
+    bad = m.copy(); bad[1] = bad[0]
+    with pytest.raises(gpu.AmrHydroError):
+        g.regrid(h1, bad)                                   # a patch named twice
+    bad = m.copy(); bad[0] = -1
+    with pytest.raises(gpu.AmrHydroError):
+        g.regrid(h1, bad)                                   # a new level-0 patch has no parent
+    bad = m.copy(); bad[0], bad[1] = m[1], m[0]
+    with pytest.raises(gpu.AmrHydroError):
+        g.regrid(h1, bad)                                   # a survivor must keep its origin
+    assert np.array_equal(g.download(0), U0)               # nothing happened
+    small = gpu.AmrHydro(h0, 1.4, 5, nslots=3)
+    with pytest.raises(gpu.AmrHydroError):
+        small.regrid(h1, m)                                 # the pool is too small
+    g.regrid(h1, m)
+    assert g.npatch == 16
