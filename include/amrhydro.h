@@ -86,6 +86,9 @@ extern "C" {
 
 #define AMRHYDRO_NBR_COARSE_FINE (-1)
 #define AMRHYDRO_NBR_PHYSICAL (-2)
+#define AMRHYDRO_NBR_REMOTE (-3)  /* patch sharding: the neighbour lives on another shard and is not mirrored in this pool;
+                                     no kernel reads or fills that region (allowed for edge/corner regions of owned
+                                     patches and for any region of a mirror patch)                                  */
 
 typedef struct amrhydro amrhydro_t;
 
@@ -166,6 +169,27 @@ int amrhydro_restrict(amrhydro_t *h, int fine_level, int fine_slot, int coarse_s
 int amrhydro_reflux(amrhydro_t *h, int coarse_level, int slot);
 
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src_slot, int dst_slot);
+
+/* Patch sharding, one shard per handle / GPU ("a grid is the basic unit"
+ * of the distribution).  Built for single-level hierarchies in direct-halo mode (AMRHYDRO_OPT_HALO = 1); the
+ * parent-child exchange of 8(e)(3) is not built.  A shard's table lists its OWNED patches first (a contiguous Morton
+ * range of the global table) and then MIRROR patches: copies of the face neighbours that other shards own.
+ *   set_owned: the kernels of every call (cfl_dt, rk_stage, ...) run on the first `owned` patches only; mirrors are data.
+ *     Every face region of an owned patch must name a patch of this pool (owned or mirror) or be physical.
+ *   set_halo_plan: send_pairs[nsend][2] = (owned patch, face), recv_pairs[nrecv][2] = (mirror patch, face): the slab
+ *     "two interior layers next to that face", [var][2][16][16] elements each, in plan order.  The sender's plan towards
+ *     a peer and the peer's receive plan list the same global (patch, face) pairs in the same order (the partitioner
+ *     sorts both by global patch index, then face), so a buffer is copied between shards as it is (cudaMemcpyPeerAsync,
+ *     ncclSend/ncclRecv or a P2P store; the tests use a device-to-device copy between two pools on one GPU).
+ *   halo_bytes(which): size of the send (0) or receive (1) buffer in bytes.
+ *   halo_pack / halo_unpack: pool -> device buffer (k_halo_slabs) / device buffer -> mirror interiors, asynchronous on
+ *     the bound stream.  One exchange of slot_in before each rk_stage; the step size is cfl dx / max over shards of the
+ *     smax that amrhydro_cfl_dt returns (allreduce(max) of one scalar). */
+int amrhydro_set_owned(amrhydro_t *h, int owned);
+int amrhydro_set_halo_plan(amrhydro_t *h, const int *send_pairs, int nsend, const int *recv_pairs, int nrecv);
+size_t amrhydro_halo_bytes(const amrhydro_t *h, int which);
+int amrhydro_halo_pack(amrhydro_t *h, int slot, void *dev_buf);
+int amrhydro_halo_unpack(amrhydro_t *h, int slot, const void *dev_buf);
 
 /* Regrid steps on either side of the hot path (PAPER.md:43-45 leaves regridding to the
  * host code; the table itself is rebuilt by the caller and handed to amrhydro_set_hierarchy).

@@ -22,7 +22,8 @@ EXPORTS = [
     "amrhydro_upload", "amrhydro_download", "amrhydro_download_padded", "amrhydro_download_registers",
     "amrhydro_cfl_dt", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
     "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_refine_indicator",
-    "amrhydro_prolong_interior", "amrhydro_regrid", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
+    "amrhydro_prolong_interior", "amrhydro_regrid", "amrhydro_set_owned", "amrhydro_set_halo_plan",
+    "amrhydro_halo_bytes", "amrhydro_halo_pack", "amrhydro_halo_unpack", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
 ]
 
 
@@ -69,6 +70,12 @@ def load_library():
     L.amrhydro_refine_indicator.argtypes = [vp, i, i, dp]
     L.amrhydro_prolong_interior.argtypes = [vp, i, i, i]
     L.amrhydro_regrid.argtypes = [vp, C.POINTER(PatchDesc), i, i, C.POINTER(C.c_int), i]
+    L.amrhydro_set_owned.argtypes = [vp, i]
+    L.amrhydro_set_halo_plan.argtypes = [vp, C.POINTER(C.c_int), i, C.POINTER(C.c_int), i]
+    L.amrhydro_halo_bytes.restype = C.c_size_t
+    L.amrhydro_halo_bytes.argtypes = [vp, i]
+    L.amrhydro_halo_pack.argtypes = [vp, i, vp]
+    L.amrhydro_halo_unpack.argtypes = [vp, i, vp]
     L.amrhydro_advance.argtypes = [vp, d, d, dp]
     L.amrhydro_advance_host.argtypes = [vp, d, d, i, vp, vp, dp]
     L.amrhydro_sync.argtypes = [vp]
@@ -127,6 +134,26 @@ class AmrHydro:
         view[:, 4] = par
         view[:, 5:32] = nbr
         return tbl
+
+    # ---- patch sharding (one shard per handle)
+    def set_owned(self, owned):
+        self._ok(self.L.amrhydro_set_owned(self.h, int(owned)))
+        self.owned = int(owned)
+
+    def set_halo_plan(self, send_pairs, recv_pairs):
+        sp = np.ascontiguousarray(send_pairs, dtype=np.int32).reshape(-1, 2)
+        rp = np.ascontiguousarray(recv_pairs, dtype=np.int32).reshape(-1, 2)
+        ip = C.POINTER(C.c_int)
+        self._ok(self.L.amrhydro_set_halo_plan(self.h, sp.ctypes.data_as(ip), len(sp), rp.ctypes.data_as(ip), len(rp)))
+
+    def halo_bytes(self, which):
+        return int(self.L.amrhydro_halo_bytes(self.h, which))
+
+    def halo_pack(self, slot, dev_ptr):
+        self._ok(self.L.amrhydro_halo_pack(self.h, slot, dev_ptr))
+
+    def halo_unpack(self, slot, dev_ptr):
+        self._ok(self.L.amrhydro_halo_unpack(self.h, slot, dev_ptr))
 
     def regrid(self, hier, old_of_new, slot=0):
         """amrhydro_regrid: the new table on the live pool (needs max_patches >= the new patch count)."""

@@ -39,6 +39,10 @@ struct amrhydro {
   int bc[6] = {0, 0, 0, 0, 0, 0};
   std::vector<amrhydro_patch_desc> tbl;
   std::vector<int> child, octant, lev_first, lev_count;
+  std::vector<int> lev_run;                 // patches of a level the kernels run on: all of them, or the owned ones of a shard
+  // patch sharding (NEXT-2): slabs this shard sends to / receives from its peers (patch * 8 + face), on the device
+  int *d_halo_send = nullptr, *d_halo_recv = nullptr;
+  int n_halo_send = 0, n_halo_recv = 0;
   std::vector<char> lev_has_cf, lev_has_phys;   // level has coarse-fine ghost regions / faces on an outflow boundary
   Desc *d_desc = nullptr;
   int *d_child = nullptr, *d_octant = nullptr;
@@ -162,6 +166,9 @@ void free_hierarchy(amrhydro *h) {
   cudaFree(h->d_desc); cudaFree(h->d_child); cudaFree(h->d_octant);
   cudaFree(h->d_Rf); cudaFree(h->d_Rc); cudaFree(h->d_bflux); cudaFree(h->d_smax);
   cudaFree(h->d_cflist); cudaFree(h->d_frtasks); cudaFree(h->d_bneed);
+  cudaFree(h->d_halo_send); cudaFree(h->d_halo_recv);
+  h->d_halo_send = h->d_halo_recv = nullptr;
+  h->n_halo_send = h->n_halo_recv = 0;
   h->d_cflist = h->d_frtasks = h->d_bneed = nullptr;
   h->d_smax = nullptr;
   h->smax_slot.clear();
@@ -323,7 +330,7 @@ static int check_table(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, in
     if (first[d.level] < 0) first[d.level] = p;
     ++count[d.level];
     for (int r = 0; r < 27; ++r)
-      if (r != 13 && (d.nbr[r] >= np || d.nbr[r] < -2 || (d.nbr[r] >= 0 && tbl[d.nbr[r]].level != d.level)))
+      if (r != 13 && (d.nbr[r] >= np || d.nbr[r] < AMRHYDRO_NBR_REMOTE || (d.nbr[r] >= 0 && tbl[d.nbr[r]].level != d.level)))
         return fail(h, AMRHYDRO_EINVAL, "bad neighbour entry");
     for (int f = 0; f < 6; ++f)                // no kernel fills a physical ghost zone on a periodic side
       if (d.nbr[face_region(f)] == AMRHYDRO_NBR_PHYSICAL && bc[f] == AMRHYDRO_BC_PERIODIC)
@@ -363,7 +370,10 @@ static int check_table(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, in
         lo0[a] = std::min(lo0[a], tbl[p].origin[a]);
         hi0[a] = std::max(hi0[a], tbl[p].origin[a] + NI);
       }
-    for (int p = 0; p < np; ++p)
+    bool shard = false;                        // a shard's table (AMRHYDRO_NBR_REMOTE entries) holds part of the domain only
+    for (int p = 0; p < np && !shard; ++p)
+      for (int r = 0; r < 27; ++r) shard |= (r != 13 && tbl[p].nbr[r] == AMRHYDRO_NBR_REMOTE);
+    for (int p = 0; p < np && !shard; ++p)
       for (int f = 0; f < 6; ++f) {
         const int a = f >> 1, l = tbl[p].level;
         const bool touches = (f & 1) ? (tbl[p].origin[a] + NI == (hi0[a] << l)) : (tbl[p].origin[a] == (lo0[a] << l));
@@ -385,6 +395,7 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
   free_hierarchy(h);
   h->tbl.assign(tbl, tbl + np);
   h->child = child; h->octant = octant; h->lev_first = first; h->lev_count = count;
+  h->lev_run = count;
   h->nlev = nlev; h->dx0 = dx0;
   for (int i = 0; i < 6; ++i) h->bc[i] = bc[i];
   h->lev_has_cf.assign(nlev, 0);
@@ -550,7 +561,7 @@ static int ensure_smax(amrhydro_t *h, int level, int slot) {
   int r = dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    k_cfl<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level],
+    k_cfl<T, NV><<<h->lev_run[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level],
                                                               make_params<T>(h), h->d_smax + level, h->d_scalars + 1);
     LAUNCH_CHECK(h);
     return 0;
@@ -608,14 +619,14 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
     constexpr int NV = decltype(nv)::value;
     if (phase1) {
       // sibling copies skipped: only the patches with a coarse-fine region have anything to fill
-      const int nb = skip ? h->cf_count[level] : h->lev_count[level];
+      const int nb = skip ? h->cf_count[level] : h->lev_run[level];
       k_fill_ghosts<T, NV><<<dim3(nb, NP), 256, 0, h->stream>>>(
           make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, skip,
           skip ? h->d_cflist + h->cf_first[level] : nullptr);
       LAUNCH_CHECK(h);
     }
     if (phase2) {
-      k_fill_outflow<T, NV><<<h->lev_count[level], 256, 0, h->stream>>>(
+      k_fill_outflow<T, NV><<<h->lev_run[level], 256, 0, h->stream>>>(
           make_pool<T>(h), slot, h->lev_first[level], h->d_desc, h->bc[0], h->bc[1], h->bc[2], h->bc[3], h->bc[4], h->bc[5]);
       LAUNCH_CHECK(h);
     }
@@ -630,7 +641,7 @@ static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot) {
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    k_fill_ghosts<T, NV><<<dim3(h->lev_count[level], NP), 256, 0, h->stream>>>(
+    k_fill_ghosts<T, NV><<<dim3(h->lev_run[level], NP), 256, 0, h->stream>>>(
         make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2, nullptr);
     LAUNCH_CHECK(h);
     return 0;
@@ -647,7 +658,7 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    const int n = h->lev_count[level], first = h->lev_first[level];
+    const int n = h->lev_run[level], first = h->lev_first[level];
     T *bflux = regs ? (T *)h->d_bflux : nullptr;
     // captured step: dt carries the exact factor 2^-level and the launches read dt0 from device memory
     const DtDev dtd = h->dt_dev ? DtDev{h->d_dt, dt, hx} : DtDev{nullptr, 0.0, 0.0};
@@ -694,7 +705,7 @@ int amrhydro_restrict(amrhydro_t *h, int flev, int fslot, int cslot) {
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    k_restrict<T, NV><<<h->lev_count[flev], 256, 0, h->stream>>>(make_pool<T>(h), fslot, cslot, h->lev_first[flev],
+    k_restrict<T, NV><<<h->lev_run[flev], 256, 0, h->stream>>>(make_pool<T>(h), fslot, cslot, h->lev_first[flev],
                                                                   h->d_desc, h->d_octant);
     LAUNCH_CHECK(h);
     return 0;
@@ -710,7 +721,7 @@ int amrhydro_reflux(amrhydro_t *h, int clev, int slot) {
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    const int nf = h->lev_count[clev + 1];
+    const int nf = h->lev_run[clev + 1];
     for (int axis = 0; axis < 3; ++axis) {
       k_reflux<T, NV><<<dim3(nf, 2), 64, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[clev + 1], 2 * axis,
                                                           h->d_desc, h->d_octant, (T *)h->d_Rf, (T *)h->d_Rc,
@@ -729,7 +740,7 @@ int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor) {
   if (!std::isfinite(factor)) return fail(h, AMRHYDRO_EINVAL, "factor must be finite");
   return dispatch(h, [&](auto t, auto nv) {          // psi does not enter the signal speeds: cached maxima stay valid
     using T = decltype(t);
-    k_scale_var<T><<<h->lev_count[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level], 8, T(factor));
+    k_scale_var<T><<<h->lev_run[level], 256, 0, h->stream>>>(make_pool<T>(h), slot, h->lev_first[level], 8, T(factor));
     LAUNCH_CHECK(h);
     (void)nv;
     return 0;
@@ -741,7 +752,7 @@ int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_o
   if (int r = check_level(h, level)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (!host_octmax) return fail(h, AMRHYDRO_EINVAL, "host_octmax is null");
-  const int n = h->lev_count[level];
+  const int n = h->lev_run[level];
   const size_t bytes = size_t(n) * 8 * sizeof(double);
   if (int r = ensure_stage(h, bytes)) return r;
   const double inv2dx = 0.5 / (h->dx0 / double(1 << level));
@@ -866,6 +877,82 @@ int amrhydro_regrid(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np_new, i
   cudaStreamSynchronize(h->stream);          // newp / d_map outlive the asynchronous copies
   cudaFree(d_map);
   return rc;
+}
+
+// ---- patch sharding: this handle holds one shard
+int amrhydro_set_owned(amrhydro_t *h, int owned) {
+  if (int r = check_ready(h)) return r;
+  if (h->nlev != 1) return fail(h, AMRHYDRO_EINVAL, "sharding is built for single-level hierarchies (no parent-child exchange yet)");
+  if (owned <= 0 || owned > h->np) return fail(h, AMRHYDRO_EINVAL, "owned patch count out of range");
+  for (int p = 0; p < owned; ++p)            // an owned patch must find all six face neighbours in this pool
+    for (int f = 0; f < 6; ++f)
+      if (h->tbl[p].nbr[face_region(f)] == AMRHYDRO_NBR_COARSE_FINE || h->tbl[p].nbr[face_region(f)] == AMRHYDRO_NBR_REMOTE)
+        return fail(h, AMRHYDRO_EINVAL, "owned patch without a face neighbour in this pool (mirror patch missing)");
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  drop_graph(h);
+  h->lev_run[0] = owned;
+  std::fill(h->smax_slot.begin(), h->smax_slot.end(), -1);
+  return 0;
+}
+
+static int upload_plan(amrhydro_t *h, const int *pairs, int n, int **dev, int *count, bool send) {
+  for (int i = 0; i < n; ++i) {
+    const int p = pairs[2 * i], f = pairs[2 * i + 1];
+    if (p < 0 || p >= h->np || f < 0 || f > 5) return fail(h, AMRHYDRO_EINVAL, "bad (patch, face) pair in the halo plan");
+    if (send ? p >= h->lev_run[0] : p < h->lev_run[0])
+      return fail(h, AMRHYDRO_EINVAL, send ? "a shard sends slabs of owned patches only" : "a shard receives into mirror patches only");
+  }
+  cudaFree(*dev);
+  *dev = nullptr;
+  *count = 0;
+  if (n == 0) return 0;
+  std::vector<int> code(n);
+  for (int i = 0; i < n; ++i) code[i] = pairs[2 * i] * 8 + pairs[2 * i + 1];
+  CUDA_TRY(h, cudaMalloc(dev, size_t(n) * sizeof(int)));
+  CUDA_TRY(h, cudaMemcpy(*dev, code.data(), size_t(n) * sizeof(int), cudaMemcpyHostToDevice));
+  *count = n;
+  return 0;
+}
+
+int amrhydro_set_halo_plan(amrhydro_t *h, const int *send_pairs, int nsend, const int *recv_pairs, int nrecv) {
+  if (int r = check_ready(h)) return r;
+  if (nsend < 0 || nrecv < 0 || (nsend && !send_pairs) || (nrecv && !recv_pairs)) return fail(h, AMRHYDRO_EINVAL, "bad halo plan");
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  if (int r = upload_plan(h, send_pairs, nsend, &h->d_halo_send, &h->n_halo_send, true)) return r;
+  return upload_plan(h, recv_pairs, nrecv, &h->d_halo_recv, &h->n_halo_recv, false);
+}
+
+size_t amrhydro_halo_bytes(const amrhydro_t *h, int which) {
+  if (!h) return 0;
+  return size_t(which ? h->n_halo_recv : h->n_halo_send) * h->nv * (NG * NI * NI) * elem(h);
+}
+
+int amrhydro_halo_pack(amrhydro_t *h, int slot, void *dev_buf) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (h->n_halo_send == 0) return 0;
+  if (!dev_buf) return fail(h, AMRHYDRO_EINVAL, "send buffer is null");
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    k_halo_slabs<T, true><<<dim3(h->n_halo_send, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, h->d_halo_send, (T *)dev_buf);
+    LAUNCH_CHECK(h);
+    (void)nv;
+    return 0;
+  });
+}
+
+int amrhydro_halo_unpack(amrhydro_t *h, int slot, const void *dev_buf) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (h->n_halo_recv == 0) return 0;
+  if (!dev_buf) return fail(h, AMRHYDRO_EINVAL, "receive buffer is null");
+  return dispatch(h, [&](auto t, auto nv) {
+    using T = decltype(t);
+    k_halo_slabs<T, false><<<dim3(h->n_halo_recv, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, h->d_halo_recv, (T *)dev_buf);
+    LAUNCH_CHECK(h);
+    (void)nv;
+    return 0;
+  });
 }
 
 int amrhydro_copy_slot(amrhydro_t *h, int level, int src, int dst) {

@@ -38,6 +38,24 @@ __global__ void __launch_bounds__(256) k_scale_var(Pool<T> pool, int slot, int f
     u[cell<T>(k + NG, j + NG, i + NG)] *= factor;
   }
 }
+// Patch sharding (NEXT-2): the two interior layers of a patch next to one of its faces, [var][2][16][16] per
+// (patch, face) entry of the plan (code = patch * 8 + face; the layer index runs along the face normal, low to high).
+// PACK: pool -> contiguous buffer on the sending shard; else buffer -> the interior of the mirror patch on the receiver.
+// One block per (entry, var).
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(256) k_halo_slabs(Pool<T> pool, int slot, const int *__restrict__ plan, T *__restrict__ buf) {
+  const int code = plan[blockIdx.x], p = code >> 3, f = code & 7, v = blockIdx.y;
+  const int d = f >> 1, lo = (f & 1) ? NI - NG : 0;
+  T *u = pool.patch(slot, p) + size_t(v) * Layout<T>::VS;
+  T *b = buf + (size_t(blockIdx.x) * pool.nv + v) * (NG * NI * NI);
+  for (int c = threadIdx.x; c < NG * NI * NI; c += 256) {
+    const int t0 = c & 15, t1 = (c >> 4) & 15, a = (c >> 8) + lo;          // two transverse indices (x fastest), layer
+    const int i = d == 0 ? a : t0, j = d == 1 ? a : (d == 0 ? t0 : t1), k = d == 2 ? a : t1;
+    const int g = cell<T>(k + NG, j + NG, i + NG);
+    if (PACK) b[c] = u[g]; else u[g] = b[c];
+  }
+}
+
 // padded box of one patch as doubles [var][20][20][20] (tests)
 template <typename T>
 __global__ void k_unpack_padded(Pool<T> pool, int slot, int p, double *__restrict__ out) {

@@ -61,3 +61,71 @@ def test_reference_arm_runs_on_rank0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+# ---------------------------------------------------------------- patch sharding: the plans of two ranks meet (NEXT-2)
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_0910_5547_b200 import sharding, workloads as wl
+    h = wl.uniform_hierarchy(4, periodic=True)
+    plan = sharding.rank_plan(h, world, rank)                          # every rank builds its own shard only
+    peer = 1 - rank
+    # a host stand-in for the slab buffers: one number per slab that names it (global patch * 8 + face), in plan order;
+    # exchange step (1) of SURVEY 8(e) as send/recv, step (2) as all_reduce(max) of one scalar
+    glob = plan["glob"]
+    send = torch.tensor([int(glob[p]) * 8 + int(f) for p, f in plan["send"][peer]], dtype=torch.int64)
+    recv = torch.zeros(len(plan["recv"][peer]), dtype=torch.int64)
+    if rank == 0:
+        dist.send(send, dst=peer); dist.recv(recv, src=peer)
+    else:
+        dist.recv(recv, src=peer); dist.send(send, dst=peer)
+    want = torch.tensor([int(glob[p]) * 8 + int(f) for p, f in plan["recv"][peer]], dtype=torch.int64)
+    smax = torch.tensor([1.0 + rank], dtype=torch.float64)
+    dist.all_reduce(smax, op=dist.ReduceOp.MAX)
+    # every slab received lands in a mirror patch, every slab sent comes from an owned one, every owned face is served
+    ok_roles = all(p >= plan["owned"] for p, _ in plan["recv"][peer]) and all(p < plan["owned"] for p, _ in plan["send"][peer])
+    nbr = plan["hier"]["nbr"]
+    served = all(nbr[p, sharding.FACE_REGION[f]] >= 0 for p in range(plan["owned"]) for f in range(6))
+    out.put((rank, bool(torch.equal(recv, want)), float(smax.item()), ok_roles, served, plan["owned"], len(recv)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharding_plans_of_two_gloo_ranks_match():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sum(r[5] for r in res) == 64
+    for rank, same, smax, roles, served, owned, nrecv in res:
+        assert same and smax == 2.0 and roles and served and nrecv > 0
+
+
+def test_partitioner_properties():
+    from paper_0910_5547_b200 import sharding, workloads as wl
+    import pytest
+    h = wl.uniform_hierarchy(4, periodic=True)
+    for ns in (1, 2, 3, 5, 8, 64):
+        R = sharding.partition_morton(h, ns)
+        assert R[0][0] == 0 and R[-1][1] == 64 and all(a[1] == b[0] for a, b in zip(R, R[1:]))
+        sizes = [hi - lo for lo, hi in R]
+        assert max(sizes) - min(sizes) <= 1
+        S = [sharding.build_shard(h, R, s) for s in range(ns)]
+        for s in range(ns):
+            for t, v in S[s]["send_global"].items():
+                assert v == S[t]["recv_global"][s]
+            assert sorted(S[s]["send"]) == sorted(S[s]["send_global"])
+    # Morton ranges are compact: with 8 shards of a 4^3 level every shard is a 2^3 cube with 24 face-neighbour mirrors
+    S = sharding.build_shard(h, sharding.partition_morton(h, 8), 3)
+    assert S["owned"] == 8 and len(S["glob"]) == 32
+    with pytest.raises(ValueError):
+        sharding.partition_morton(wl.ball_hierarchy(2, 2), 2)
+    with pytest.raises(ValueError):
+        sharding.partition_morton(h, 65)
