@@ -13,7 +13,8 @@
 // Every function follows the paper's order and notation; the readings taken where
 // PAPER.md is garbled (G1-G6) or silent (S1-S21) are those of SURVEY.md section 8(c)
 // (S17-S21: DESIGN.md section 3) and are listed again in DESIGN.md.  Pins: tests/test_oracle_*.py
-// (P1-P12 the hot path, P13-P17 the 9-variable GLM system, P18-P19 the regrid steps).
+// (P1-P12 the hot path, P13-P17 the 9-variable GLM system, P18-P19 the regrid steps, P20 the floors of S11,
+// P21 the global time step on several levels).
 // Parity unpinned: none of the per-step functions (all have at least one pin);
 // the long-time Brio-Wu / Sedov / KH *profiles* have no printed values in the paper.
 //

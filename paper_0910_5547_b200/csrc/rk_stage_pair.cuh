@@ -222,7 +222,7 @@ __device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P
 #ifdef AMR_PK_MAXNREG        // tuning: an explicit register cap instead of the one implied by CTAs per SM
 #define AMR_PK_BOUNDS __maxnreg__(AMR_PK_MAXNREG)
 #else
-#define AMR_PK_BOUNDS __launch_bounds__(pk::THREADS, AMR_PK_MINB)
+#define AMR_PK_BOUNDS __launch_bounds__(pk::THREADS, (sizeof(T) == 4 ? AMR_PK_MINB + 1 : AMR_PK_MINB))   // fp32: three CTAs per SM (<= 168 registers)
 #endif
 template <typename T, int NV, bool BASE>
 __global__ void AMR_PK_BOUNDS
