@@ -93,7 +93,7 @@ extern "C" {
 typedef struct amrhydro amrhydro_t;
 
 /* One row of the patch-descriptor table (128 bytes).  Patches must be sorted by level.
- * origin: index of the first interior cell on the patch's own level (multiple of 16).
+ * origin: index of the first interior cell on the patch's own level (multiple of patch_dim).
  * parent: patch id on level-1 whose octant this patch refines (-1 on level 0).
  * nbr[r], r = (dz+1)*9 + (dy+1)*3 + (dx+1): id of the same-level patch at block offset
  * (dx,dy,dz) (periodic wrap is expressed here), AMRHYDRO_NBR_COARSE_FINE or
@@ -106,8 +106,16 @@ typedef struct amrhydro_patch_desc {
 } amrhydro_patch_desc;
 
 /* Create a solver context.  gamma: adiabatic index of Eq. 6, > 1.
- * nvars in {5, 8, 9}; patch_dim must be 16 and nghost 2 (BASELINE.json north_star; the stencil
- * i-2..i+1 of PAPER.md:104).  Returns NULL on a bad argument or when no CUDA device exists. */
+ * nvars in {5, 8, 9}; nghost must be 2 (the stencil i-2..i+1 of PAPER.md:104); patch_dim is 16 (BASELINE.json
+ * north_star) or 32, 48, 64 ("arbitrary grid dimensions can arise").  A patch of
+ * (16 s)^3 cells is held as s^3 patches of 16^3: the scheme is defined on cells and sibling halos are exact copies, so
+ * the result does not depend on the decomposition (tests/test_gpu_patchdim.py: bitwise the 16^3 run).  With
+ * patch_dim > 16: descriptor origins are multiples of patch_dim, a fine patch is an octant of its parent as before,
+ * parents and neighbours follow from level, origin and the boundary conditions (the nbr entries of the caller's table are
+ * not read), host data is [patch][var][D][D][D], max_patches and patch ranges count the caller's patches, and the calls
+ * that address single 16^3 patches (download_padded, download_registers, refine_indicator, prolong_interior, regrid,
+ * set_owned, set_halo_plan) return AMRHYDRO_EINVAL.  Other patch shapes, direct flux reconstruction and higher order
+ * are not built.  Returns NULL on a bad argument or when no CUDA device exists. */
 amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost);
 void amrhydro_destroy(amrhydro_t *h);
 const char *amrhydro_last_error(const amrhydro_t *h);

@@ -91,7 +91,7 @@ class AmrHydro:
     """One solver context + pool.  Method names mirror the C ABI (amrhydro_<name>)."""
 
     def __init__(self, hier, gamma, nvars, dtype="f64", theta=1.5, nslots=None, kernel=3, halo=1,
-                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2, graph=0, max_patches=None):
+                 rho_floor=1e-30, e_floor=1e-30, device="cuda:0", stream=None, fuse_cfl=2, ch=1.0, cr=0.18, zsplit=2, graph=0, max_patches=None, patch_dim=None):
         import torch  # device memory + streams only
         if not torch.cuda.is_available():
             raise AmrHydroError("no CUDA device: the amrhydro path has no CPU fallback")
@@ -99,7 +99,8 @@ class AmrHydro:
         self.torch = torch
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.h = self.L.amrhydro_create(gamma, nvars, 16, 2)
+        self.pdim = int(patch_dim or hier.get("ni", 16))          # 16, or 32 / 48 / 64 (held as 16^3 sub-patches by the library)
+        self.h = self.L.amrhydro_create(gamma, nvars, self.pdim, 2)
         if not self.h:
             raise AmrHydroError("amrhydro_create failed (bad arguments or no device)")
         self.nv = nvars
@@ -198,7 +199,7 @@ class AmrHydro:
 
     def download(self, slot, first=0, count=None):
         count = self.npatch - first if count is None else count
-        out = np.empty((count, self.nv, 16, 16, 16), dtype=self.np_dtype)
+        out = np.empty((count, self.nv, self.pdim, self.pdim, self.pdim), dtype=self.np_dtype)
         self._ok(self.L.amrhydro_download(self.h, slot, first, count, out.ctypes.data))
         return out
 

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <string>
 #include <type_traits>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/amrhydro.h"
@@ -26,6 +27,9 @@ static_assert(sizeof(amrhydro_patch_desc) == 128 && sizeof(Desc) == 128, "descri
 struct amrhydro {
   double gamma = 1.4;
   int nv = 5, bits = 64;
+  // NEXT-4: patches of 32^3, 48^3, 64^3 cells are held as sub^3 patches of 16^3 (the scheme is defined on cells; sibling
+  // halos are exact copies, so the decomposition does not change a bit of the result); np_user counts the caller's patches
+  int pdim = NI, sub = 1, nsub = 1, np_user = 0;
   double theta = 1.5, rho_floor = 1e-30, e_floor = 1e-30;
   double glm_ch = 1.0, glm_cr = 0.18;      // S17, S18 (nvars = 9)
   int kernel = 3, halo = 1;                 // rk_stage_pair for nvars = 5 (rk_stage_march otherwise); direct sibling halos
@@ -185,12 +189,17 @@ extern "C" {
 static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot);
 
 amrhydro_t *amrhydro_create(double gamma, int nvars, int patch_dim, int nghost) {
-  if (!(gamma > 1.0) || (nvars != 5 && nvars != 8 && nvars != 9) || patch_dim != NI || nghost != NG) return nullptr;
+  if (!(gamma > 1.0) || (nvars != 5 && nvars != 8 && nvars != 9) || patch_dim < NI || patch_dim > 4 * NI || patch_dim % NI ||
+      nghost != NG)
+    return nullptr;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return nullptr;   // no CPU fallback
   amrhydro *h = new amrhydro;
   h->gamma = gamma;
   h->nv = nvars;
+  h->pdim = patch_dim;
+  h->sub = patch_dim / NI;
+  h->nsub = h->sub * h->sub * h->sub;
   {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
@@ -294,7 +303,7 @@ int amrhydro_get_counter(amrhydro_t *h, int key, long long *out, int reset) {
 
 size_t amrhydro_pool_bytes(const amrhydro_t *h, int max_patches, int nslots) {
   if (!h || max_patches <= 0 || nslots <= 0) return 0;
-  return size_t(nslots) * size_t(max_patches) * size_t(h->nv) * vs(h) * elem(h);
+  return size_t(nslots) * size_t(max_patches) * size_t(h->nsub) * size_t(h->nv) * vs(h) * elem(h);
 }
 
 int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patches, int nslots, void *stream) {
@@ -304,6 +313,7 @@ int amrhydro_bind_pool(amrhydro_t *h, void *dev_pool, size_t bytes, int max_patc
   if (bytes < need) return fail(h, AMRHYDRO_ENOMEM, "pool smaller than amrhydro_pool_bytes()");
   if ((uintptr_t)dev_pool % 256) return fail(h, AMRHYDRO_EINVAL, "pool must be 256-byte aligned");
   drop_graph(h);
+  max_patches *= h->nsub;                    // from here on in 16^3 patches
   h->pool = dev_pool; h->pool_bytes = bytes; h->maxp = max_patches; h->nslots = nslots;
   h->stream = (cudaStream_t)stream;
   h->bound = true;
@@ -385,7 +395,7 @@ static int check_table(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, in
   return 0;
 }
 
-int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
+static int install_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
   if (int r = check_ready(h, false)) return r;
   if (!tbl || !bc || np <= 0 || nlev <= 0 || !(dx0 > 0)) return fail(h, AMRHYDRO_EINVAL, "bad hierarchy arguments");
   if (np > h->maxp) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
@@ -463,15 +473,97 @@ int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np
     h->bflux_patches = mx;
   }
   h->np = np;
+  h->np_user = np / h->nsub;
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));   // the pageable-memory copies above are staged: make them final
   return 0;
+}
+
+// patch_dim = 16 s, s > 1 (NEXT-4): the caller's table of (16 s)^3 patches becomes a table of 16^3 patches, s^3 per
+// patch in (z, y, x) order right after one another, so that internal patch = user patch * s^3 + sub-index and levels stay
+// contiguous.  Parents and the 27 neighbour entries follow from level, origin and the boundary conditions alone (periodic
+// wrap over the extent of level 0); the caller's nbr entries are not read.
+static int expand_table(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, const int *bc,
+                        std::vector<amrhydro_patch_desc> &out) {
+  const int D = h->pdim, S = h->sub, NS = h->nsub;
+  auto key = [](int l, int x, int y, int z) {
+    return (uint64_t(l) << 60) | (uint64_t(x) << 40) | (uint64_t(y) << 20) | uint64_t(z);
+  };
+  int lo0[3] = {1 << 30, 1 << 30, 1 << 30}, hi0[3] = {-(1 << 30), -(1 << 30), -(1 << 30)};
+  for (int p = 0; p < np; ++p) {
+    const auto &d = tbl[p];
+    if (d.level < 0 || d.level >= nlev) return fail(h, AMRHYDRO_EINVAL, "patch level out of range");
+    if (p > 0 && d.level < tbl[p - 1].level) return fail(h, AMRHYDRO_EINVAL, "patches must be sorted by level");
+    for (int a = 0; a < 3; ++a) {
+      if (d.origin[a] < 0 || d.origin[a] % D || d.origin[a] >= (1 << 20)) return fail(h, AMRHYDRO_EINVAL, "origin must be a multiple of patch_dim");
+      if (d.level == 0) { lo0[a] = std::min(lo0[a], d.origin[a]); hi0[a] = std::max(hi0[a], d.origin[a] + D); }
+    }
+    if (d.level == 0 && d.parent != -1) return fail(h, AMRHYDRO_EINVAL, "level-0 patches have parent -1");
+    if (d.level > 0) {
+      const int Q = d.parent;
+      if (Q < 0 || Q >= np || tbl[Q].level != d.level - 1) return fail(h, AMRHYDRO_EINVAL, "bad parent");
+      for (int a = 0; a < 3; ++a) {
+        const int rel = d.origin[a] - 2 * tbl[Q].origin[a];
+        if (rel != 0 && rel != D) return fail(h, AMRHYDRO_EINVAL, "patch is not an octant of its parent");
+      }
+    }
+  }
+  if (tbl[0].level != 0) return fail(h, AMRHYDRO_EINVAL, "empty level");
+  std::unordered_map<uint64_t, int> id;
+  id.reserve(size_t(np) * NS * 2);
+  out.assign(size_t(np) * NS, amrhydro_patch_desc{});
+  for (int p = 0; p < np; ++p)
+    for (int s = 0; s < NS; ++s) {
+      const int sx = s % S, sy = (s / S) % S, sz = s / (S * S), q = p * NS + s;
+      out[q].level = tbl[p].level;
+      out[q].origin[0] = tbl[p].origin[0] + NI * sx;
+      out[q].origin[1] = tbl[p].origin[1] + NI * sy;
+      out[q].origin[2] = tbl[p].origin[2] + NI * sz;
+      if (!id.emplace(key(out[q].level, out[q].origin[0], out[q].origin[1], out[q].origin[2]), q).second)
+        return fail(h, AMRHYDRO_EINVAL, "two patches cover the same cells");
+    }
+  for (auto &d : out) {
+    d.parent = -1;
+    if (d.level > 0) {
+      auto it = id.find(key(d.level - 1, (d.origin[0] / 2) / NI * NI, (d.origin[1] / 2) / NI * NI, (d.origin[2] / 2) / NI * NI));
+      if (it == id.end()) return fail(h, AMRHYDRO_EINVAL, "bad parent");
+      d.parent = it->second;
+    }
+    for (int r = 0; r < 27; ++r) {
+      const int off[3] = {r % 3 - 1, (r / 3) % 3 - 1, r / 9 - 1};
+      int q[3];
+      bool outside = false;
+      for (int a = 0; a < 3; ++a) {
+        q[a] = d.origin[a] + NI * off[a];
+        const int lo = lo0[a] << d.level, hi = hi0[a] << d.level;
+        if (q[a] < lo || q[a] >= hi) {
+          if (bc[2 * a + (q[a] >= hi ? 1 : 0)] == AMRHYDRO_BC_PERIODIC) q[a] = lo + ((q[a] - lo) % (hi - lo) + (hi - lo)) % (hi - lo);
+          else outside = true;
+        }
+      }
+      if (outside) { d.nbr[r] = AMRHYDRO_NBR_PHYSICAL; continue; }
+      auto it = id.find(key(d.level, q[0], q[1], q[2]));
+      d.nbr[r] = it == id.end() ? AMRHYDRO_NBR_COARSE_FINE : it->second;
+    }
+  }
+  return 0;
+}
+
+int amrhydro_set_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np, int nlev, double dx0, const int *bc) {
+  if (!h) return AMRHYDRO_EINVAL;
+  if (h->sub == 1) return install_hierarchy(h, tbl, np, nlev, dx0, bc);
+  if (int r = check_ready(h, false)) return r;
+  if (!tbl || !bc || np <= 0 || nlev <= 0 || !(dx0 > 0)) return fail(h, AMRHYDRO_EINVAL, "bad hierarchy arguments");
+  if (size_t(np) * h->nsub > size_t(h->maxp)) return fail(h, AMRHYDRO_ENOMEM, "more patches than the pool holds");
+  std::vector<amrhydro_patch_desc> sub;
+  if (int r = expand_table(h, tbl, np, nlev, bc, sub)) return r;
+  return install_hierarchy(h, sub.data(), int(sub.size()), nlev, dx0, bc);
 }
 
 int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *host) {
   if (int r = check_ready(h)) return r;
   if (int r = check_slot(h, slot)) return r;
-  if (!host || first < 0 || count < 0 || first + count > h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
-  const size_t per = size_t(h->nv) * 4096 * elem(h);
+  if (!host || first < 0 || count < 0 || first + count > h->np_user) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  const size_t per = size_t(h->nv) * h->pdim * h->pdim * h->pdim * elem(h);        // one of the caller's patches
   const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
   if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
   for (int l = 0; l < h->nlev; ++l) smax_touch(h, l, slot);
@@ -481,7 +573,8 @@ int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *h
                                 cudaMemcpyHostToDevice, h->stream));
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      k_pack<T><<<dim3(n, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, first + done, (const T *)h->d_stage);
+      k_pack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (const T *)h->d_stage,
+                                                                 h->sub);
       LAUNCH_CHECK(h);
       (void)nv;
       return 0;
@@ -494,15 +587,16 @@ int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *h
 int amrhydro_download(amrhydro_t *h, int slot, int first, int count, void *host) {
   if (int r = check_ready(h)) return r;
   if (int r = check_slot(h, slot)) return r;
-  if (!host || first < 0 || count < 0 || first + count > h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
-  const size_t per = size_t(h->nv) * 4096 * elem(h);
+  if (!host || first < 0 || count < 0 || first + count > h->np_user) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  const size_t per = size_t(h->nv) * h->pdim * h->pdim * h->pdim * elem(h);
   const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
   if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
   for (int done = 0; done < count; done += chunk) {
     int n = std::min(chunk, count - done);
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      k_unpack<T><<<dim3(n, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, first + done, (T *)h->d_stage);
+      k_unpack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (T *)h->d_stage,
+                                                                   h->sub);
       LAUNCH_CHECK(h);
       (void)nv;
       return 0;
@@ -517,6 +611,7 @@ int amrhydro_download(amrhydro_t *h, int slot, int first, int count, void *host)
 
 int amrhydro_download_padded(amrhydro_t *h, int slot, int patch, double *out) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (int r = check_slot(h, slot)) return r;
   if (!out || patch < 0 || patch >= h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch");
   size_t bytes = size_t(h->nv) * NP * NP * NP * sizeof(double);
@@ -537,6 +632,7 @@ int amrhydro_download_padded(amrhydro_t *h, int slot, int patch, double *out) {
 
 int amrhydro_download_registers(amrhydro_t *h, int patch, double *rf, double *rc) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (!rf || !rc || patch < 0 || patch >= h->np) return fail(h, AMRHYDRO_EINVAL, "bad patch");
   size_t n = size_t(6) * h->nv * 64;
   if (!h->d_Rf) { std::fill(rf, rf + n, 0.0); std::fill(rc, rc + n, 0.0); return 0; }
@@ -749,6 +845,7 @@ int amrhydro_glm_damp(amrhydro_t *h, int level, int slot, double factor) {
 
 int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_octmax) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (int r = check_level(h, level)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (!host_octmax) return fail(h, AMRHYDRO_EINVAL, "host_octmax is null");
@@ -772,6 +869,7 @@ int amrhydro_refine_indicator(amrhydro_t *h, int level, int slot, double *host_o
 
 int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slot) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (check_slot(h, slot) || check_slot(h, parent_slot)) return AMRHYDRO_EINVAL;
   if (patch < 0 || patch >= h->np || h->tbl[patch].level == 0) return fail(h, AMRHYDRO_EINVAL, "patch has no parent");
   smax_touch(h, h->tbl[patch].level, slot);
@@ -786,6 +884,7 @@ int amrhydro_prolong_interior(amrhydro_t *h, int patch, int slot, int parent_slo
 
 int amrhydro_regrid(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np_new, int nlev_new, const int *old_of_new, int slot) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (int r = check_slot(h, slot)) return r;
   if (!tbl || !old_of_new || np_new <= 0 || nlev_new <= 0) return fail(h, AMRHYDRO_EINVAL, "bad regrid arguments");
   if (h->nslots < 2) return fail(h, AMRHYDRO_ESTATE, "regrid needs a second slot as scratch");
@@ -882,6 +981,7 @@ int amrhydro_regrid(amrhydro_t *h, const amrhydro_patch_desc *tbl, int np_new, i
 // ---- patch sharding: this handle holds one shard
 int amrhydro_set_owned(amrhydro_t *h, int owned) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (h->nlev != 1) return fail(h, AMRHYDRO_EINVAL, "sharding is built for single-level hierarchies (no parent-child exchange yet)");
   if (owned <= 0 || owned > h->np) return fail(h, AMRHYDRO_EINVAL, "owned patch count out of range");
   for (int p = 0; p < owned; ++p)            // an owned patch must find all six face neighbours in this pool
@@ -916,6 +1016,7 @@ static int upload_plan(amrhydro_t *h, const int *pairs, int n, int **dev, int *c
 
 int amrhydro_set_halo_plan(amrhydro_t *h, const int *send_pairs, int nsend, const int *recv_pairs, int nrecv) {
   if (int r = check_ready(h)) return r;
+  if (h->sub != 1) return fail(h, AMRHYDRO_EINVAL, "this call addresses 16^3 patches: patch_dim = 16 only");
   if (nsend < 0 || nrecv < 0 || (nsend && !send_pairs) || (nrecv && !recv_pairs)) return fail(h, AMRHYDRO_EINVAL, "bad halo plan");
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   if (int r = upload_plan(h, send_pairs, nsend, &h->d_halo_send, &h->n_halo_send, true)) return r;
@@ -1063,10 +1164,10 @@ int amrhydro_advance_host(amrhydro_t *h, double cfl, double dt_fixed, int nsteps
                           double *dt_last) {
   if (int r = check_ready(h)) return r;
   if (!host_in || !host_out || nsteps < 0) return fail(h, AMRHYDRO_EINVAL, "bad host buffers");
-  if (int r = amrhydro_upload(h, 0, 0, h->np, host_in)) return r;
+  if (int r = amrhydro_upload(h, 0, 0, h->np_user, host_in)) return r;
   for (int s = 0; s < nsteps; ++s)
     if (int r = amrhydro_advance(h, cfl, dt_fixed, dt_last)) return r;
-  return amrhydro_download(h, 0, 0, h->np, host_out);
+  return amrhydro_download(h, 0, 0, h->np_user, host_out);
 }
 
 int amrhydro_sync(amrhydro_t *h) {

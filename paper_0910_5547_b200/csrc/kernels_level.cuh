@@ -8,25 +8,31 @@
 namespace amr {
 
 // ------------------------------------------------------------------ staging <-> pool
-// staging: [count][var][16][16][16] (host interior layout).  One block per (patch, var).
+// staging: [count][var][D][D][D] (host interior layout), D = 16 S: the caller's patch.  One block per (16^3 patch, var);
+// with S > 1 the block's patch is sub-block (sz, sy, sx) = s of the caller's patch p / S^3 (NEXT-4).
+template <typename T> __device__ __forceinline__ size_t stage_base(int p, int v, int nv, int S) {
+  const int NS = S * S * S, u = p / NS, s = p % NS, D = NI * S;
+  const int sx = s % S, sy = (s / S) % S, sz = s / (S * S);
+  return ((size_t(u) * nv + v) * D + sz * NI) * D * D + size_t(sy * NI) * D + sx * NI;
+}
 template <typename T>
-__global__ void __launch_bounds__(256) k_pack(Pool<T> pool, int slot, int first, const T *__restrict__ stage) {
-  const int p = blockIdx.x, v = blockIdx.y;
+__global__ void __launch_bounds__(256) k_pack(Pool<T> pool, int slot, int first, const T *__restrict__ stage, int S) {
+  const int p = blockIdx.x, v = blockIdx.y, D = NI * S;
   T *dst = pool.patch(slot, first + p) + size_t(v) * Layout<T>::VS;
-  const T *src = stage + (size_t(p) * pool.nv + v) * (NI * NI * NI);
+  const T *src = stage + stage_base<T>(p, v, pool.nv, S);
   for (int c = threadIdx.x; c < NI * NI * NI; c += 256) {
     int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
-    dst[cell<T>(k + NG, j + NG, i + NG)] = src[c];
+    dst[cell<T>(k + NG, j + NG, i + NG)] = src[(size_t(k) * D + j) * D + i];
   }
 }
 template <typename T>
-__global__ void __launch_bounds__(256) k_unpack(Pool<T> pool, int slot, int first, T *__restrict__ stage) {
-  const int p = blockIdx.x, v = blockIdx.y;
+__global__ void __launch_bounds__(256) k_unpack(Pool<T> pool, int slot, int first, T *__restrict__ stage, int S) {
+  const int p = blockIdx.x, v = blockIdx.y, D = NI * S;
   const T *src = pool.patch(slot, first + p) + size_t(v) * Layout<T>::VS;
-  T *dst = stage + (size_t(p) * pool.nv + v) * (NI * NI * NI);
+  T *dst = stage + stage_base<T>(p, v, pool.nv, S);
   for (int c = threadIdx.x; c < NI * NI * NI; c += 256) {
     int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
-    dst[c] = src[cell<T>(k + NG, j + NG, i + NG)];
+    dst[(size_t(k) * D + j) * D + i] = src[cell<T>(k + NG, j + NG, i + NG)];
   }
 }
 // interior cells of one variable times a factor (S18: psi <- psi exp(-dt c_h / c_r))

@@ -27,7 +27,7 @@ def _morton(b):
     return key
 
 
-def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton"):
+def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton", ni=NI):
     """Flat descriptor table of a block-structured hierarchy (refinement ratio 2).
 
     base_blocks: (nbx, nby, nbz) level-0 patches per axis (all exist).
@@ -35,6 +35,7 @@ def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton
              (block b covers cells [16 b, 16 b + 16) of the level); each must be an octant
              of an existing patch one level down.
     bc: per face (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi): 0 periodic, 1 outflow.
+    ni: cells per patch side (16; 32, 48, 64 for amrhydro_create's larger patch_dim).
     Returns dict(level, origin, parent, nbr, nlevels, dx0, bc, blocks).
     nbr[p][r], r=(dz+1)*9+(dy+1)*3+(dx+1): >=0 same-level patch, -1 coarse-fine, -2 physical.
     """
@@ -64,7 +65,7 @@ def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton
             p = ids[l][b]
             level[p] = l
             blocks[p] = b
-            origin[p] = [NI * x for x in b]
+            origin[p] = [ni * x for x in b]
             if l > 0:
                 pb = tuple(x >> 1 for x in b)
                 if pb not in ids[l - 1]:
@@ -83,8 +84,8 @@ def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton
                             outside = True
                 nbr[p, r] = -2 if outside else ids[l].get(tuple(q), -1)
     h = dict(level=level, origin=origin, parent=parent, nbr=nbr, nlevels=len(levels),
-             dx0=float(box) / (NI * base_blocks[0]), bc=np.asarray(bc, np.int32), blocks=blocks,
-             base_blocks=base_blocks)
+             dx0=float(box) / (ni * base_blocks[0]), bc=np.asarray(bc, np.int32), blocks=blocks,
+             base_blocks=base_blocks, ni=ni)
     _check_nesting(h)
     return h
 
@@ -99,7 +100,7 @@ def _check_nesting(h):
             if h["nbr"][p, FACE_REGION[f]] != -1:
                 continue
             d, hi = f // 2, f & 1
-            rel = (h["origin"][p, d] - 2 * h["origin"][Q, d]) // NI  # octant bit along d
+            rel = (h["origin"][p, d] - 2 * h["origin"][Q, d]) // h.get("ni", NI)  # octant bit along d
             on_parent_face = (rel == 1) if hi else (rel == 0)
             if on_parent_face and h["nbr"][Q, FACE_REGION[f]] < 0:
                 raise ValueError("improper nesting at patch %d face %d" % (p, f))
@@ -161,16 +162,17 @@ def level_patches(h, l):
 def cell_centres(h, p):
     """(x, y, z) 1-D arrays of the interior cell centres of patch p (unit box)."""
     dx = h["dx0"] / (1 << int(h["level"][p]))
-    return tuple((h["origin"][p, d] + np.arange(NI) + 0.5) * dx for d in range(3))
+    return tuple((h["origin"][p, d] + np.arange(h.get("ni", NI)) + 0.5) * dx for d in range(3))
 
 
 def split_global(h, G, l=0):
-    """Cut a global [nv][nz][ny][nx] array of level l into [npatch_l][nv][16][16][16]."""
+    """Cut a global [nv][nz][ny][nx] array of level l into [npatch_l][nv][ni][ni][ni] (ni = 16 unless the hierarchy says otherwise)."""
     ps = level_patches(h, l)
-    out = np.empty((len(ps), G.shape[0], NI, NI, NI), G.dtype)
+    ni = h.get("ni", NI)
+    out = np.empty((len(ps), G.shape[0], ni, ni, ni), G.dtype)
     for n, p in enumerate(ps):
         ox, oy, oz = h["origin"][p]
-        out[n] = G[:, oz:oz + NI, oy:oy + NI, ox:ox + NI]
+        out[n] = G[:, oz:oz + ni, oy:oy + ni, ox:ox + ni]
     return out
 
 
