@@ -158,7 +158,11 @@ int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_o
 
 /* a2: fill the ghost zones of every patch of `level` in `slot` (S5): same-level copy where
  * nbr >= 0; conservative limited-linear prolongation (S6) of (1-alpha)*parent_old_slot +
- * alpha*parent_new_slot (S7) where nbr == -1; zero-gradient outflow where nbr == -2. */
+ * alpha*parent_new_slot (S7) where nbr == -1; zero-gradient outflow where nbr == -2.
+ * With AMRHYDRO_OPT_HALO = 1 (direct sibling reads) the sibling copies are made only on levels someone prolongates from; on the
+ * finest level this call writes just what rk_stage reads from a patch's own ghost zone: the six face slabs
+ * that lie on a coarse-fine or physical boundary.  Edge and corner regions next to a coarse-fine boundary of
+ * a finest-level patch are then left as they are. */
 int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int parent_old_slot,
                          int parent_new_slot, double alpha);
 

@@ -171,9 +171,19 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   const int *nbr = D.nbr + (oz + 1) * 9;             // the nine regions of this plane
   bool cf = false;                                   // block-uniform: does this plane touch a coarse-fine region?
   const bool skip_siblings = mode & 1;
+  // faces_only (sibling copies skipped = direct halos on the finest level): only the six face slabs are read by anyone
+  // (rk_stage), so edge and corner regions are left alone and the parent tile is loaded only where a
+  // face slab prolongates from it
+  const bool faces_only = skip_siblings;
+  bool fxl = false, fxh = false, fyl = false, fyh = false;
   if (Q >= 0 && !(mode & 2)) {
+    if (faces_only) {
+      if (oz != 0) cf = nbr[4] == -1;
+      else { fxl = nbr[3] == -1; fxh = nbr[5] == -1; fyl = nbr[1] == -1; fyh = nbr[7] == -1; cf = fxl | fxh | fyl | fyh; }
+    } else {
 #pragma unroll
-    for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
+      for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
+    }
   }
   int pc0[3] = {0, 0, 0};                            // parent padded index of the tile's first cell
   if (cf) {
@@ -185,12 +195,18 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
     const bool only_old = alpha == T(0), only_new = alpha == T(1);
     // 432 tile cells per variable over 256 threads: two cells per thread, their parent offsets computed once
     const int r0 = threadIdx.x, r1 = threadIdx.x + 256;
-    const int c0 = cell<T>(pc0[2] + r0 / (CT * CT), pc0[1] + (r0 / CT) % CT, pc0[0] + r0 % CT);
-    const int c1 = r1 < CTV ? cell<T>(pc0[2] + r1 / (CT * CT), pc0[1] + (r1 / CT) % CT, pc0[0] + r1 % CT) : -1;
+    // (faces_only, interior plane: a tile cell is needed if it lies within the three coarse columns / rows of a face slab)
+    auto needed = [&](int r) {
+      if (!faces_only || oz != 0) return true;
+      const int tx = r % CT, ty = (r / CT) % CT;
+      return (fxl && tx <= 2) || (fxh && tx >= CT - 3) || (fyl && ty <= 2) || (fyh && ty >= CT - 3);
+    };
+    const int c0 = needed(r0) ? cell<T>(pc0[2] + r0 / (CT * CT), pc0[1] + (r0 / CT) % CT, pc0[0] + r0 % CT) : -1;
+    const int c1 = r1 < CTV && needed(r1) ? cell<T>(pc0[2] + r1 / (CT * CT), pc0[1] + (r1 / CT) % CT, pc0[0] + r1 % CT) : -1;
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const T *po = Co + size_t(v) * Layout<T>::VS, *pn = Cn + size_t(v) * Layout<T>::VS;
-      s_par[v * CTV + r0] = only_old ? po[c0] : (only_new ? pn[c0] : (T(1) - alpha) * po[c0] + alpha * pn[c0]);
+      if (c0 >= 0) s_par[v * CTV + r0] = only_old ? po[c0] : (only_new ? pn[c0] : (T(1) - alpha) * po[c0] + alpha * pn[c0]);
       if (c1 >= 0) s_par[v * CTV + r1] = only_old ? po[c1] : (only_new ? pn[c1] : (T(1) - alpha) * po[c1] + alpha * pn[c1]);
     }
   }
@@ -222,6 +238,7 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
     locate(t, i, j);
     const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
     if (nbr[(oy + 1) * 3 + (ox + 1)] != -1) continue;
+    if (faces_only && (ox != 0) + (oy != 0) + (oz != 0) != 1) continue;      // edge / corner region: nobody reads it
     const int pad[3] = {i, j, k};
     int c0 = 0;
     T s[3];
