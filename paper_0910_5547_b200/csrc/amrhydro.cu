@@ -696,7 +696,15 @@ int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_o
   return 0;
 }
 
+// stage_only: the caller knows that only rk_stage will read these ghosts (the fill of U1 before the combination stage
+// inside amrhydro_advance): with direct halos that needs the coarse-fine / physical face slabs and nothing else, on any level
+static int fill_ghosts_impl(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha, bool stage_only);
+
 int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha) {
+  return fill_ghosts_impl(h, level, slot, pold, pnew, alpha, false);
+}
+
+static int fill_ghosts_impl(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha, bool stage_only) {
   if (int r = check_ready(h)) return r;
   if (int r = check_level(h, level)) return r;
   if (int r = check_slot(h, slot)) return r;
@@ -707,7 +715,7 @@ int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew,
     pold = pnew = slot;
   }
   // direct-halo mode: sibling copies are only needed where someone prolongates from this level
-  const int skip = (h->halo == 1 && level + 1 >= h->nlev) ? 1 : 0;   // (mode bit 0 of k_fill_ghosts)
+  const int skip = (h->halo == 1 && (level + 1 >= h->nlev || stage_only)) ? 1 : 0;   // (mode bit 0 of k_fill_ghosts)
   const bool phase1 = !skip || h->lev_has_cf[level], phase2 = h->lev_has_phys[level];
   if (!phase1 && !phase2) return 0;   // e.g. periodic single level with direct halos: nothing to materialise
   return dispatch(h, [&](auto t, auto nv) {
@@ -1078,7 +1086,7 @@ static int advance_level(amrhydro_t *h, int lev, double dt, double a1, double a2
   if ((r = amrhydro_fill_ghosts(h, lev, 0, 2, 0, a1))) return r;
   if (kids && (r = amrhydro_copy_slot(h, lev, 0, 2))) return r;
   if ((r = amrhydro_rk_stage(h, lev, 0, 0, 1, 0.0, 1.0, dt, w))) return r;      // U1 = Un + dt L(Un)
-  if ((r = amrhydro_fill_ghosts(h, lev, 1, 2, 0, a2))) return r;
+  if ((r = fill_ghosts_impl(h, lev, 1, 2, 0, a2, true))) return r;              // (U1's ghosts are read by the next line only)
   if ((r = amrhydro_rk_stage(h, lev, 1, 0, 0, 0.5, 0.5, dt, w))) return r;      // Un+1 = (Un + U1 + dt L(U1))/2
   if (h->nv == 9 && h->glm_cr > 0.0 &&                                           // S18
       (r = amrhydro_glm_damp(h, lev, 0, std::exp(-dt * h->glm_ch / h->glm_cr)))) return r;
