@@ -4,11 +4,19 @@
 One "step" = one pass of the whole hot path over one level/hierarchy: CFL reduction, ghost
 fill, RK stage 1, ghost fill, RK stage 2 (plus restriction/refluxing on AMR workloads).
 Default workload: BASELINE.json configs[4] (512^3 uniform periodic Euler stress test, 32768
-patches of 16^3), the configuration the metric is quoted on.  Inputs are seeded and synthetic
-(paper_0910_5547_b200/workloads.py).  Prints ONE JSON line on rank 0.
+patches of 16^3), the configuration the metric is quoted on, in fp64; the same workload in fp32
+is timed right after it and reported as the sub-record "fp32" of the same JSON line (the
+configuration names both precisions).  Inputs are seeded and synthetic
+(paper_0910_5547_b200/workloads.py).  Prints ONE JSON line on rank 0: value (device-resident),
+e2e (host buffers through amrhydro_advance_host), roofline of the stage kernel (algorithmic
+bytes / CUDA-event time / measured HBM peak, plus the ncu DRAM bytes and the issue / FP64-pipe
+fractions), cpu_baseline (the oracle on the host cores), clocks (NVML samples in the timed region).
+--workload cfg3 (AMR) runs amrhydro_advance as one CUDA-graph replay per coarse step.
+--gpus N (torchrun): N independent replicas, weak scaling, max-over-ranks timing.
+--impl reference: the CPU oracle on a bounded sample (there is no reference implementation).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--impl ours|reference]
-                  [--workload cfg5|cfg2|cfg4|cfg3] [--size S] [--halo 0|1]
+                  [--workload cfg5|cfg2|cfg4|cfg4g|cfg3] [--size S] [--halo 0|1] [--graph 0|1] [--no-fp32]
 """
 import argparse
 import json

@@ -269,27 +269,23 @@ template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18, 
 #ifndef AMR_BASE_TMA
 #define AMR_BASE_TMA 1      // combination stage: U_base planes come through their own TMA ring (no global loads in the warps)
 #endif
-// LITE: register-light layout for two CTAs per SM (rk_stage_lite.cuh): 3-slot ring, the flux
-// arrays alias the q+ arrays (slot s is read as q+ by its only reader before that same thread
-// overwrites it with the flux), plus per-thread slots for the z-marching state.
-template <typename T, int NV, bool LITE = false, bool WB = true> struct Smem {   // WB: the kernel reads U_base (combination stage)
-  static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY, NSLOT = LITE ? 3 : Cfg<T>::NSLOT;
+template <typename T, int NV, bool WB = true> struct Smem {   // WB: the kernel reads U_base (combination stage)
+  static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY, NSLOT = Cfg<T>::NSLOT;
   static constexpr int RAWP = NV * NI * NI;        // one raw plane: [NV][16][16], dense TMA box
   static constexpr int WV = NP * PW;               // one variable of one primitive plane [20][PW]
   static constexpr int QXV = NI * PQ;              // [16][PQ]: slot s = q+ of cell s-1 / flux at face s
   static constexpr int QYV = (NI + 1) * PY;        // [17][PY]
-  static constexpr int ACV = NI * NI;              // per-thread slots, indexed by (warp, lane)
-  // the flux arrays alias the q+ arrays in LITE, and in the fp64 MHD combination stage so that its U_base ring fits
-  static constexpr bool ALIAS = LITE || (WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 8);
+  // the flux arrays alias the q+ arrays (slot s is read as q+ by its only reader before that same thread overwrites it
+  // with the flux) in the fp64 MHD combination stage, so that its U_base ring fits
+  static constexpr bool ALIAS = WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 8;
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
                        O_FX = ALIAS ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
-                       O_FY = ALIAS ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV,
-                       O_QPZ = O_ACC + (LITE ? NV * ACV : 0);
+                       O_FY = ALIAS ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV;
   // ring of U_base planes for the combination stage (128-byte aligned TMA destination).  fp32 Euler: the extra
   // 20 kB cost the third CTA per SM, so that instantiation also takes 96 registers instead of 64 (launch bounds)
-  static constexpr int O_BRAW = ((O_QPZ + (LITE ? NV * ACV : 0) + 31) / 32) * 32;
-  static constexpr bool BTMA = !LITE && WB && AMR_BASE_TMA && (sizeof(T) == 8 || NV == 5) &&
-                               size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, fp64 MHD does not)
+  static constexpr int O_BRAW = ((O_ACC + 31) / 32) * 32;
+  static constexpr bool BTMA = WB && AMR_BASE_TMA && (sizeof(T) == 8 || NV == 5) &&
+                               size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, fp64 GLM-9 does not)
   static constexpr int O_END = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
   static constexpr size_t BYTES = BAR_OFF + NSLOT * 8 + 128;   // + slack to align the ring to 128 B
@@ -413,7 +409,7 @@ __global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
                  const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd) {
-  using S = mk::Smem<T, NV, false, BASE>;
+  using S = mk::Smem<T, NV, BASE>;
   if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
   constexpr int PX = Layout<T>::PX, PLANE = Layout<T>::PLANE, VS = Layout<T>::VS, LEAD = Layout<T>::LEAD;
@@ -657,7 +653,7 @@ int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sb
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
                           cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
   static bool configured = false;
-  constexpr size_t bytes0 = mk::Smem<T, NV, false, false>::BYTES, bytes1 = mk::Smem<T, NV, false, true>::BYTES;
+  constexpr size_t bytes0 = mk::Smem<T, NV, false>::BYTES, bytes1 = mk::Smem<T, NV, true>::BYTES;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
     if (e == cudaSuccess)

@@ -11,15 +11,21 @@
 //    chains (ILP 2); the x face between them never leaves the registers; all own-cell and y-direction
 //    shared-memory accesses are 16-byte (fp64) / 8-byte (fp32) vectors: about half the LDS/STS
 //    instructions per cell; the update is stored with 16-byte stores.
+//  * the x exchange (q+ of cell 2px+1 to the right neighbour, flux through face 2px to the left one) is a warp
+//    shuffle inside the 8 lanes of a row; shared memory carries only the patch edge (q+ of the ghost cell -1,
+//    q+ of cell 15 / flux through face 16) and the y exchange.
 //  * no halo warps: each of the 128 threads also converts ONE of the 128 halo cells of a plane
-//    (loaded one plane ahead straight from the sibling's interior or the own ghost zone), and the
-//    ghost-cell slopes + the fluxes through faces 16 are two full-warp passes per plane that rotate
-//    over the four warps.
+//    (loaded one plane ahead straight from the sibling's interior or the own ghost zone); the ghost-cell
+//    slopes (one warp pass per direction) and the fluxes through faces 16 (ONE warp pass for x and y, the
+//    direction a run-time value of the lane) rotate over the four warps.
+//  * CTA barriers are mbarrier arrive / wait halves with independent work between them (z slopes, z fluxes and
+//    the update of the cell below after the first arrive; the conversion of plane c+2 after the second).
 //  * the flux arrays alias the q+ arrays (a slot is read as q+ by its only reader before that same
-//    thread overwrites it with its flux), U_base rides on a 2-slot TMA ring of its own: 91-113 kB of
-//    shared memory per CTA (fp64 Euler), so that two CTAs fit an SM in both stages.
+//    thread overwrites it with its flux), U_base rides on a 2-slot TMA ring of its own: 87-107 kB of
+//    shared memory per CTA (fp64 Euler), so that two CTAs fit an SM in both stages (fp32: three).
 // Results are those of k_rk_stage_march up to the rounding of c = q_{i+1} - q_{i-1} (taken directly,
-// as the oracle does, in x and y).
+// as the oracle does, in x and y).  Measured alternatives (a warp-specialised split, other plane orders, one
+// cell per thread with twice the warps) are in profiles/README.md; all were slower.
 #pragma once
 #include "rk_stage_march.cuh"
 
@@ -39,9 +45,6 @@ template <typename T> __device__ __forceinline__ void st2(T *p, T x, T y) {
 }
 
 constexpr int THREADS = 128;
-#ifndef AMR_PK_XSHFL
-#define AMR_PK_XSHFL 1     // x exchange (q+ to the right neighbour, flux to the left one) through warp shuffles; shared memory only at the patch edge
-#endif
 
 // 64-bit shuffles inside the 8 lanes of one row (lane = (row & 3) * 8 + px)
 __device__ __forceinline__ double shfl_up8(double x) { return __shfl_up_sync(0xffffffffu, x, 1, 8); }
@@ -55,11 +58,7 @@ template <typename T, int NV, bool WB> struct Smem {
   static constexpr int RAWP = NV * NI * NI;        // one raw plane [NV][16][16], dense TMA box
   static constexpr int PW = NP;                    // primitive plane [20][20]: even pitch, pairs are 16-byte aligned
   static constexpr int WV = NP * PW;
-#if AMR_PK_XSHFL
   static constexpr int QXP = 1, QXV = 2 * NI;      // [2][16 rows]: column 0 = q+ of cell -1, column 1 = q+ of cell 15 / flux through face 16
-#else
-  static constexpr int QXP = 9, QXV = NI * QXP;    // [16 rows][9]: slot t = q+ of cell 2t-1 / flux through face 2t
-#endif
   static constexpr int QYV = (NI + 1) * NI;        // [17][16]: slot j = q+ of row j-1 / flux through face j
   static constexpr int HQV = 16;                   // q- of the ghost cell 16 of every line (per direction)
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
@@ -136,7 +135,7 @@ __device__ __forceinline__ void halo_slopes(T *sm, int buf, int lane, T th2) {
   const int t = lane & 15, hi = lane >> 4;
   const T *s3 = sm + S::O_W + buf * (NV * WV) +
                 (D == 0 ? (t + NG) * PW + (hi ? NG + NI - 1 : 0) : (hi ? NG + NI - 1 : 0) * PW + (t + NG));
-  T *qlo = sm + (D == 0 ? S::O_QX + t * S::QXP : S::O_QY + t);      // (QXP = 1 with AMR_PK_XSHFL: column 0)
+  T *qlo = sm + (D == 0 ? S::O_QX + t * S::QXP : S::O_QY + t);      // (column 0 of the x edge array)
   T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
   constexpr int qv = D == 0 ? S::QXV : S::QYV;
 #pragma unroll
@@ -154,7 +153,7 @@ __device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T
   if (lane >= 16) return;
   const int t = lane;
   constexpr int qv = D == 0 ? S::QXV : S::QYV;
-  T *q16 = sm + (D == 0 ? S::O_QX + (AMR_PK_XSHFL ? NI + t : t * S::QXP + 8) : S::O_QY + NI * NI + t);
+  T *q16 = sm + (D == 0 ? S::O_QX + (NI + t) : S::O_QY + NI * NI + t);
   const T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
   T WL[NV], WR[NV], G[NV];
 #pragma unroll
@@ -172,9 +171,6 @@ __device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T
 // both at once (Euler): lanes 0-15 the x faces, lanes 16-31 the y faces, with the direction a run-time value of the
 // lane.  Same operations in the same order as mk::face_flux<T, 0> / <T, 1> (B * v is written fma(B, v, 0), which rounds
 // identically), so a face shared by two patches still gets bitwise the same flux from both.
-#ifndef AMR_PK_HFLUX1
-#define AMR_PK_HFLUX1 1
-#endif
 template <typename T>
 __device__ __forceinline__ void face_flux_xy(const T (&L)[5], const T (&R)[5], const Params<T> &P, T (&G)[5], bool y) {
   const T rl = L[0], el = L[1], rr = R[0], er = R[1];
@@ -199,7 +195,7 @@ __device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P
   constexpr int NV = 5;
   const int t = lane & 15, d = lane >> 4;
   const int qv = d ? S::QYV : S::QXV;
-  T *q16 = sm + (d ? S::O_QY + NI * NI + t : S::O_QX + (AMR_PK_XSHFL ? NI + t : t * S::QXP + 8));
+  T *q16 = sm + (d ? S::O_QY + NI * NI + t : S::O_QX + (NI + t));
   const T *hq = sm + S::O_HQ + d * (NV * S::HQV) + t;
   T WL[NV], WR[NV], G[NV];
 #pragma unroll
@@ -219,11 +215,7 @@ __device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P
 #ifndef AMR_PK_MINB
 #define AMR_PK_MINB 2
 #endif
-#ifdef AMR_PK_MAXNREG        // tuning: an explicit register cap instead of the one implied by CTAs per SM
-#define AMR_PK_BOUNDS __maxnreg__(AMR_PK_MAXNREG)
-#else
 #define AMR_PK_BOUNDS __launch_bounds__(pk::THREADS, (sizeof(T) == 4 ? AMR_PK_MINB + 1 : AMR_PK_MINB))   // fp32: three CTAs per SM (<= 168 registers)
-#endif
 template <typename T, int NV, bool BASE>
 __global__ void AMR_PK_BOUNDS
 k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
@@ -307,11 +299,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   T *out = pool.patch(sout, p) + off;
   const T *raw = sm + S::O_RAW + j * NI + i0;                 // this pair in ring slot 0, v = 0
   T *wme = sm + S::O_W + (j + NG) * PW + (i0 + NG);           // this pair in primitive buffer 0, v = 0
-#if AMR_PK_XSHFL
   T *qx = sm + S::O_QX + j + (px == 7 ? NI : 0);              // px = 0: q+ of cell -1 of this row; px = 7: q+ of cell 15 / flux through face 16
-#else
-  T *qx = sm + S::O_QX + j * S::QXP + px;                     // slot px: q+ of cell i0-1 / flux through face i0
-#endif
   T *qy = sm + S::O_QY + j * NI + i0;                         // slot j: q+ of row j-1 / flux through face j
 
   T Uh[NV];                                                   // halo cell of the next plane to convert
@@ -389,9 +377,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 #pragma unroll
     for (int v = 0; v < NV; ++v) { const auto x = pk::ld2(w + v * WV); Wc[0][v] = x.x; Wc[1][v] = x.y; }
     T qmx0[NV], qpx0[NV], qmx1[NV], qmy0[NV], qmy1[NV];
-#if AMR_PK_XSHFL
     T WLs[NV];                                     // q+ of cell i0-1 from the left neighbour's registers (px > 0)
-#endif
     if (live) {
       // 1. slopes of both cells along x and y; publish the q+ the neighbours need
 #pragma unroll
@@ -405,13 +391,9 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         qmx0[v] = fma(-qs, mr, a0); qpx0[v] = fma(qs, mr, a0);
         mr = pk::slope_mr(d1, d2, wr - a0, th2, qs);
         qmx1[v] = fma(-qs, mr, a1);
-#if AMR_PK_XSHFL
         const T qpx1 = fma(qs, mr, a1);
         WLs[v] = pk::shfl_up8(qpx1);
         if (px == 7) qx[v * QXV] = qpx1;           // for the flux through face 16 (halo_flux)
-#else
-        qx[v * QXV + 1] = fma(qs, mr, a1);
-#endif
         mr = pk::slope_mr(a0 - wd.x, wu.x - a0, wu.x - wd.x, th2, qs);
         qmy0[v] = fma(-qs, mr, a0);
         const T qpy0 = fma(qs, mr, a0);
@@ -420,7 +402,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
       }
       if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
-      if (warp == ((c + (AMR_PK_HFLUX1 ? 1 : 2)) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
+      if (warp == ((c + 1) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
       arrive(0);
     }
     // 2. z (between the two halves of the barrier): slope of cell c from this pair's own planes c-1 (dzm), c, c+1;
@@ -497,12 +479,8 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       T WL[NV], WD0[NV], WD1[NV];
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
-#if AMR_PK_XSHFL
         WL[v] = WLs[v];
         if (px == 0) WL[v] = qx[v * QXV];          // q+ of the ghost cell -1 (halo_slopes)
-#else
-        WL[v] = qx[v * QXV];
-#endif
         const auto y = pk::ld2(qy + v * QYV);
         WD0[v] = y.x; WD1[v] = y.y;
       }
@@ -512,18 +490,10 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
       mk::face_flux<T, 1>(WD1, qmy1, P, Gy1);
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
-#if !AMR_PK_XSHFL
-        qx[v * QXV] = Gx0[v];
-#endif
         pk::st2(qy + v * QYV, Gy0[v], Gy1[v]);
       }
     }
-#if AMR_PK_HFLUX1
     if (warp == ((c + 2) & 3)) pk::halo_flux_xy<T, S>(sm, lane, P, bflux, pl, c - NG + zlo, bmask);
-#else
-    if (warp == (c & 3)) pk::halo_flux<T, NV, 0, S>(sm, lane, P, bflux, pl, c - NG + zlo);
-    if (warp == ((c + 2) & 3)) pk::halo_flux<T, NV, 1, S>(sm, lane, P, bflux, pl, c - NG + zlo);
-#endif
     arrive(1);
     if (bmask) {
       if ((i0 & 7) == 0 && ((bmask >> (i0 >> 3)) & 1)) {
@@ -553,12 +523,8 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
     // 5. flux differences in x and y, minus the low z face parked in acc
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-#if AMR_PK_XSHFL
       T fxh = pk::shfl_down8(Gx0[v]);               // flux through face i0+2 = the right neighbour's low face
       if (px == 7) fxh = qx[v * QXV];               // face 16 (halo_flux)
-#else
-      const T fxh = qx[v * QXV + 1];
-#endif
       const auto fyh = pk::ld2(qy + v * QYV + NI);
       acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) - acc[0][v];
       acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) - acc[1][v];
@@ -581,10 +547,7 @@ int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sba
                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0},
                          const int *bneed = nullptr) {
   static bool configured = false;
-#ifndef AMR_PAIR_EXTRA_SMEM
-#define AMR_PAIR_EXTRA_SMEM 0     // experiment: pad the allocation to force one CTA per SM
-#endif
-  constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES + AMR_PAIR_EXTRA_SMEM, bytes1 = pk::Smem<T, NV, true>::BYTES + AMR_PAIR_EXTRA_SMEM;
+  constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES, bytes1 = pk::Smem<T, NV, true>::BYTES;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_rk_stage_pair<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
     if (e == cudaSuccess)
