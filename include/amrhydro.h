@@ -155,6 +155,12 @@ int amrhydro_download_registers(amrhydro_t *h, int patch, double *host_fine, dou
  * reduction in the last bit.  The pool is private: data written into it behind the library's back
  * is not seen. */
 int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_out, double *smax_out);
+/* The same without the host read ("a _device variant that leaves dt in device memory is allowed for graph
+ * capture"): *dt_dev points at two doubles in the handle's device memory, written asynchronously on the bound stream by
+ * k_dt0: [0] = cfl * dx_level_first / max over levels level_first..level_last of the signal speed of `slot` (S4: with
+ * level_first = 0 and level_last = nlevels - 1 the dt0 of amrhydro_advance), [1] = 1 if that maximum is zero, NaN or inf,
+ * else 0.  Valid until the next amrhydro_cfl_dt_device / amrhydro_advance of this handle.  Does not synchronise. */
+int amrhydro_cfl_dt_device(amrhydro_t *h, int level_first, int level_last, int slot, double cfl, const double **dt_dev);
 
 /* a2: fill the ghost zones of every patch of `level` in `slot` (S5): same-level copy where
  * nbr >= 0; conservative limited-linear prolongation (S6) of (1-alpha)*parent_old_slot +

@@ -20,7 +20,7 @@ EXPORTS = [
     "amrhydro_create", "amrhydro_destroy", "amrhydro_last_error", "amrhydro_set_option",
     "amrhydro_get_counter", "amrhydro_pool_bytes", "amrhydro_bind_pool", "amrhydro_set_hierarchy",
     "amrhydro_upload", "amrhydro_download", "amrhydro_download_padded", "amrhydro_download_registers",
-    "amrhydro_cfl_dt", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
+    "amrhydro_cfl_dt", "amrhydro_cfl_dt_device", "amrhydro_fill_ghosts", "amrhydro_rk_stage", "amrhydro_restrict",
     "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_refine_indicator",
     "amrhydro_prolong_interior", "amrhydro_regrid", "amrhydro_set_owned", "amrhydro_set_halo_plan",
     "amrhydro_halo_bytes", "amrhydro_halo_pack", "amrhydro_halo_unpack", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
@@ -61,6 +61,7 @@ def load_library():
     L.amrhydro_download_padded.argtypes = [vp, i, i, dp]
     L.amrhydro_download_registers.argtypes = [vp, i, dp, dp]
     L.amrhydro_cfl_dt.argtypes = [vp, i, i, d, dp, dp]
+    L.amrhydro_cfl_dt_device.argtypes = [vp, i, i, i, d, C.POINTER(vp)]
     L.amrhydro_fill_ghosts.argtypes = [vp, i, i, i, i, d]
     L.amrhydro_rk_stage.argtypes = [vp, i, i, i, i, d, d, d, d]
     L.amrhydro_restrict.argtypes = [vp, i, i, i]
@@ -219,6 +220,12 @@ class AmrHydro:
         dt, s = C.c_double(0), C.c_double(0)
         self._ok(self.L.amrhydro_cfl_dt(self.h, level, slot, cfl, C.byref(dt), C.byref(s)))
         return dt.value
+
+    def cfl_dt_device(self, level_first, level_last, slot, cfl):
+        """Device address of (dt, non-finite flag); nothing is synchronised."""
+        out = C.c_void_p(0)
+        self._ok(self.L.amrhydro_cfl_dt_device(self.h, level_first, level_last, slot, cfl, C.byref(out)))
+        return out.value
 
     def max_speed(self, level, slot=0):
         dt, s = C.c_double(0), C.c_double(0)

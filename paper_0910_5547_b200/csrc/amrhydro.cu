@@ -700,6 +700,20 @@ int amrhydro_cfl_dt(amrhydro_t *h, int level, int slot, double cfl, double *dt_o
 // inside amrhydro_advance): with direct halos that needs the coarse-fine / physical face slabs and nothing else, on any level
 static int fill_ghosts_impl(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha, bool stage_only);
 
+int amrhydro_cfl_dt_device(amrhydro_t *h, int level_first, int level_last, int slot, double cfl, const double **dt_dev) {
+  if (int r = check_ready(h)) return r;
+  if (int r = check_level(h, level_first)) return r;
+  if (int r = check_level(h, level_last)) return r;
+  if (int r = check_slot(h, slot)) return r;
+  if (level_last < level_first || !dt_dev) return fail(h, AMRHYDRO_EINVAL, "bad level range or null output");
+  for (int l = level_first; l <= level_last; ++l)
+    if (int r = ensure_smax(h, l, slot)) return r;
+  k_dt0<<<1, 32, 0, h->stream>>>(h->d_smax, level_first, level_last, cfl * (h->dx0 / double(1 << level_first)), 0.0, h->d_dt);
+  LAUNCH_CHECK(h);
+  *dt_dev = h->d_dt;
+  return 0;
+}
+
 int amrhydro_fill_ghosts(amrhydro_t *h, int level, int slot, int pold, int pnew, double alpha) {
   return fill_ghosts_impl(h, level, slot, pold, pnew, alpha, false);
 }

@@ -79,3 +79,31 @@ def test_graph_reports_non_finite_speed(gpu):
     g.upload(0, U)
     with pytest.raises(gpu.AmrHydroError):
         g.advance(0.3)
+
+
+def test_cfl_dt_device_leaves_dt_on_the_device(gpu):
+    """amrhydro_cfl_dt_device: the same number as amrhydro_cfl_dt, bit for bit, without a host read (read back here with
+    a plain cudaMemcpy), for one level and as the dt0 of a whole hierarchy (S4); the flag reports a NaN."""
+    cudart = pytest.importorskip("cuda.cudart")
+    import ctypes
+
+    def read(ptr):
+        buf = (ctypes.c_double * 2)()
+        err, = cudart.cudaMemcpy(ctypes.addressof(buf), ptr, 16, cudart.cudaMemcpyKind.cudaMemcpyDeviceToHost)
+        assert int(err) == 0
+        return buf[0], buf[1]
+
+    h = wl.ball_hierarchy(2, 3, bc=(1,) * 6)
+    U = state(h, 5, 9)
+    g = gpu.AmrHydro(h, 1.4, 5)
+    g.upload(0, U)
+    for lev in range(3):
+        dt, flag = read(g.cfl_dt_device(lev, lev, 0, 0.3))
+        assert flag == 0.0 and dt == g.cfl_dt(lev, 0, 0.3)
+    dt0, flag = read(g.cfl_dt_device(0, 2, 0, 0.3))
+    assert flag == 0.0 and dt0 == g.advance(0.3)                   # the step amrhydro_advance takes
+    U[5, 0, 1, 2, 3] = np.nan
+    g.upload(0, U)
+    assert read(g.cfl_dt_device(0, 2, 0, 0.3))[1] == 1.0
+    with pytest.raises(gpu.AmrHydroError):
+        g.cfl_dt_device(2, 1, 0, 0.3)
