@@ -228,7 +228,22 @@ template <typename T, int NV> __device__ __forceinline__ T max_speed_fast(const 
     const T m1 = ax > ay ? ax : ay;
     return (m1 > az ? m1 : az) + fsqrt(P.gg1 * W[1]);
   } else {
-    return max_signal_speed<T, NV>(W, P);
+    // S3 along the three directions with the MUFU-seeded reciprocal and square root of this file (the stand-alone
+    // k_cfl keeps the IEEE forms of physics.cuh: six IEEE square roots and a division per cell are ~170 instructions)
+    const T a2 = P.gg1 * W[1], ir = frcp(W[0]);
+    const T B2 = fma(W[7 % NV], W[7 % NV], fma(W[6 % NV], W[6 % NV], W[5 % NV] * W[5 % NV]));
+    const T s = fma(B2, ir, a2), s2 = s * s, a4 = T(4) * a2 * ir;
+    T best = T(0);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const T Bd = W[(5 + d) % NV];
+      const T disc = fma(-a4 * Bd, Bd, s2);
+      const T sq = disc > T(1e-30) * s2 ? fsqrt(disc) : T(0);
+      const T sp = tabs(W[2 + d]) + fsqrt(T(0.5) * (s + sq));
+      best = sp > best ? sp : best;
+    }
+    if (NV == 9) best = best > P.ch ? best : P.ch;                // S17
+    return best;
   }
 }
 
