@@ -65,6 +65,10 @@ struct amrhydro {
   int fuse_cfl = 2;                         // 0 never, 1 / 2 = the combination stage also reduces the max signal speed
   void *d_stage = nullptr;
   size_t stage_bytes = 0;
+  // upload / download move a range in chunks through two halves of the staging buffer: the host copy of one chunk runs on
+  // copy_stream while k_pack / k_unpack of the other runs on the bound stream
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_packed[2] = {nullptr, nullptr}, ev_entry = nullptr;
   long long launches = 0;
   // amrhydro_advance as one CUDA graph (AMRHYDRO_OPT_GRAPH): dt0 lives in d_dt, the S9 recursion is captured once per
   // hierarchy / option set and replayed; the host-side bookkeeping a replay skips is restored from the capture
@@ -154,6 +158,17 @@ int ensure_stage(amrhydro *h, size_t bytes) {
   return 0;
 }
 
+int ensure_copy_stream(amrhydro *h) {
+  if (h->copy_stream) return 0;
+  CUDA_TRY(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) {
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_packed[i], cudaEventDisableTiming));
+  }
+  CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_entry, cudaEventDisableTiming));
+  return 0;
+}
+
 // cached max signal speed of (level, slot) goes stale when interior cells of the slot are written
 void smax_touch(amrhydro *h, int level, int slot) {
   if (level >= 0 && level < (int)h->smax_slot.size() && h->smax_slot[level] == slot) h->smax_slot[level] = -1;
@@ -220,6 +235,12 @@ void amrhydro_destroy(amrhydro_t *h) {
   cudaFree(h->d_scalars);
   cudaFree(h->d_dt);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->copy_stream) {
+    cudaStreamSynchronize(h->copy_stream);
+    cudaStreamDestroy(h->copy_stream);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(h->ev_copied[i]); cudaEventDestroy(h->ev_packed[i]); }
+    cudaEventDestroy(h->ev_entry);
+  }
   cudaFree(h->d_stage);
   delete h;
 }
@@ -563,23 +584,32 @@ int amrhydro_upload(amrhydro_t *h, int slot, int first, int count, const void *h
   if (int r = check_ready(h)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (!host || first < 0 || count < 0 || first + count > h->np_user) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  if (count == 0) return 0;
   const size_t per = size_t(h->nv) * h->pdim * h->pdim * h->pdim * elem(h);        // one of the caller's patches
   const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
-  if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
+  const int nbuf = count > chunk ? 2 : 1;
+  if (int r = ensure_stage(h, size_t(nbuf) * chunk * per)) return r;
+  if (int r = ensure_copy_stream(h)) return r;
   for (int l = 0; l < h->nlev; ++l) smax_touch(h, l, slot);
-  for (int done = 0; done < count; done += chunk) {
-    int n = std::min(chunk, count - done);
-    CUDA_TRY(h, cudaMemcpyAsync(h->d_stage, (const char *)host + size_t(done) * per, size_t(n) * per,
-                                cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(h, cudaEventRecord(h->ev_entry, h->stream));            // the staging buffer may still be read by earlier work
+  CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->ev_entry, 0));
+  int it = 0;
+  for (int done = 0; done < count; done += chunk, ++it) {
+    const int n = std::min(chunk, count - done), b = it & 1;
+    char *buf = (char *)h->d_stage + size_t(b) * chunk * per;
+    if (it >= 2) CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->ev_packed[b], 0));   // k_pack of chunk it-2 has drained this half
+    CUDA_TRY(h, cudaMemcpyAsync(buf, (const char *)host + size_t(done) * per, size_t(n) * per, cudaMemcpyHostToDevice, h->copy_stream));
+    CUDA_TRY(h, cudaEventRecord(h->ev_copied[b], h->copy_stream));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0));
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      k_pack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (const T *)h->d_stage,
-                                                                 h->sub);
+      k_pack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (const T *)buf, h->sub);
       LAUNCH_CHECK(h);
       (void)nv;
       return 0;
     });
     if (r) return r;
+    CUDA_TRY(h, cudaEventRecord(h->ev_packed[b], h->stream));
   }
   return 0;
 }
@@ -588,23 +618,31 @@ int amrhydro_download(amrhydro_t *h, int slot, int first, int count, void *host)
   if (int r = check_ready(h)) return r;
   if (int r = check_slot(h, slot)) return r;
   if (!host || first < 0 || count < 0 || first + count > h->np_user) return fail(h, AMRHYDRO_EINVAL, "bad patch range");
+  if (count == 0) return 0;
   const size_t per = size_t(h->nv) * h->pdim * h->pdim * h->pdim * elem(h);
   const int chunk = int(std::max<size_t>(1, std::min<size_t>(count, (size_t(256) << 20) / per)));
-  if (int r = ensure_stage(h, size_t(chunk) * per)) return r;
-  for (int done = 0; done < count; done += chunk) {
-    int n = std::min(chunk, count - done);
+  const int nbuf = count > chunk ? 2 : 1;
+  if (int r = ensure_stage(h, size_t(nbuf) * chunk * per)) return r;
+  if (int r = ensure_copy_stream(h)) return r;
+  int it = 0;
+  for (int done = 0; done < count; done += chunk, ++it) {
+    const int n = std::min(chunk, count - done), b = it & 1;
+    char *buf = (char *)h->d_stage + size_t(b) * chunk * per;
+    if (it >= 2) CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0));       // the host copy of chunk it-2 has drained this half
     int r = dispatch(h, [&](auto t, auto nv) {
       using T = decltype(t);
-      k_unpack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (T *)h->d_stage,
-                                                                   h->sub);
+      k_unpack<T><<<dim3(n * h->nsub, h->nv), 256, 0, h->stream>>>(make_pool<T>(h), slot, (first + done) * h->nsub, (T *)buf, h->sub);
       LAUNCH_CHECK(h);
       (void)nv;
       return 0;
     });
     if (r) return r;
-    CUDA_TRY(h, cudaMemcpyAsync((char *)host + size_t(done) * per, h->d_stage, size_t(n) * per,
-                                cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaEventRecord(h->ev_packed[b], h->stream));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->copy_stream, h->ev_packed[b], 0));
+    CUDA_TRY(h, cudaMemcpyAsync((char *)host + size_t(done) * per, buf, size_t(n) * per, cudaMemcpyDeviceToHost, h->copy_stream));
+    CUDA_TRY(h, cudaEventRecord(h->ev_copied[b], h->copy_stream));
   }
+  CUDA_TRY(h, cudaStreamSynchronize(h->copy_stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   return 0;
 }

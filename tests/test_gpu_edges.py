@@ -175,3 +175,22 @@ def test_periodic_conservation_on_the_gpu_over_many_steps(gpu):
     assert np.isfinite(R).all() and g.get_counter(gpu.CNT_FLOOR_HITS) == 0
     assert (np.abs(R.sum(axis=(0, 2, 3, 4)) - t0) <= 2e-14 * scale).all()
     assert np.abs(R - U).max() > 1e-2                    # it did evolve
+
+
+def test_upload_download_round_trip_over_several_staging_chunks(gpu):
+    """Ranges larger than the 256 MB staging chunk go through two alternating halves of the staging buffer (host copy of one
+    chunk beside k_pack / k_unpack of the other): 4096 fp64 patches = 3 chunks, 5000 fp32 patches = 2, bit for bit, also
+    for a sub-range that starts inside the second chunk."""
+    for dtype, nb in (("f64", (16, 16, 16)), ("f32", (20, 25, 10))):
+        h = wl.build_hierarchy(nb, (), (0,) * 6)
+        n = len(h["level"])
+        rng = np.random.default_rng(5)
+        U = rng.standard_normal((n, 5, 16, 16, 16)).astype(np.float64 if dtype == "f64" else np.float32)
+        g = gpu.AmrHydro(h, 1.4, 5, dtype=dtype, nslots=1)
+        g.upload(0, U)
+        assert np.array_equal(g.download(0), U)
+        V = rng.standard_normal((1900, 5, 16, 16, 16)).astype(U.dtype)
+        g.upload(0, V, first=1700)
+        U[1700:3600] = V
+        assert np.array_equal(g.download(0, 1650, 2000), U[1650:3650])
+        del g
