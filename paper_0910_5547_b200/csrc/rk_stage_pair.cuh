@@ -59,7 +59,11 @@ template <typename T, int NV, bool WB> struct Smem {
   static constexpr int PW = NP;                    // primitive plane [20][20]: even pitch, pairs are 16-byte aligned
   static constexpr int WV = NP * PW;
   static constexpr int QXP = 1, QXV = 2 * NI;      // [2][16 rows]: column 0 = q+ of cell -1, column 1 = q+ of cell 15 / flux through face 16
-  static constexpr int QYV = (NI + 1) * NI;        // [17][16]: slot j = q+ of row j-1 / flux through face j
+  // fp32: a warp owns rows w, w+4, w+8, w+12 and the y array has pitch 20 (see the thread mapping in the kernel): measured
+  // 5.55 -> 5.37 ms at 512^3; fp64 (16 bytes per lane, one row per wavefront anyway) keeps rows 4w..4w+3: 10.55 vs 10.84 ms
+  static constexpr bool ROWS4 = sizeof(T) == 4;
+  static constexpr int PY = ROWS4 ? NP : NI;       // pitch of the y exchange array
+  static constexpr int QYV = (NI + 1) * PY;        // [17][PY]: slot j = q+ of row j-1 / flux through face j
   static constexpr int HQV = 16;                   // q- of the ghost cell 16 of every line (per direction)
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
                        O_QY = ((O_QX + NV * QXV + 1) / 2) * 2, O_HQ = O_QY + NV * QYV,
@@ -147,27 +151,6 @@ __device__ __forceinline__ void halo_slopes(T *sm, int buf, int lane, T th2) {
     else qlo[v * qv] = fma(qs, mr, w1);
   }
 }
-// flux through face 16 of every line (lanes 0-15), after the q+ of cell 15 has been published
-template <typename T, int NV, int D, typename S>
-__device__ __forceinline__ void halo_flux(T *sm, int lane, const Params<T> &P, T *__restrict__ bflux, int pl, int zface) {
-  if (lane >= 16) return;
-  const int t = lane;
-  constexpr int qv = D == 0 ? S::QXV : S::QYV;
-  T *q16 = sm + (D == 0 ? S::O_QX + (NI + t) : S::O_QY + NI * NI + t);
-  const T *hq = sm + S::O_HQ + D * (NV * S::HQV) + t;
-  T WL[NV], WR[NV], G[NV];
-#pragma unroll
-  for (int v = 0; v < NV; ++v) { WL[v] = q16[v * qv]; WR[v] = hq[v * S::HQV]; }
-  mk::face_flux<T, D>(WL, WR, P, G);
-#pragma unroll
-  for (int v = 0; v < NV; ++v) q16[v * qv] = G[v];
-  if (bflux) {
-    T *B = bflux + ((size_t(pl) * 9 + 3 * D + 2) * NV) * 256 + zface * 16 + t;
-#pragma unroll
-    for (int v = 0; v < NV; ++v) B[v * 256] = T(0.5) * G[v];
-  }
-}
-
 // both at once (Euler): lanes 0-15 the x faces, lanes 16-31 the y faces, with the direction a run-time value of the
 // lane.  Same operations in the same order as mk::face_flux<T, 0> / <T, 1> (B * v is written fma(B, v, 0), which rounds
 // identically), so a face shared by two patches still gets bitwise the same flux from both.
@@ -195,7 +178,7 @@ __device__ __forceinline__ void halo_flux_xy(T *sm, int lane, const Params<T> &P
   constexpr int NV = 5;
   const int t = lane & 15, d = lane >> 4;
   const int qv = d ? S::QYV : S::QXV;
-  T *q16 = sm + (d ? S::O_QY + NI * NI + t : S::O_QX + (NI + t));
+  T *q16 = sm + (d ? S::O_QY + NI * S::PY + t : S::O_QX + (NI + t));
   const T *hq = sm + S::O_HQ + d * (NV * S::HQV) + t;
   T WL[NV], WR[NV], G[NV];
 #pragma unroll
@@ -237,7 +220,10 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   const int zlo = int(blockIdx.x & zsplit) * (NI / 2), nz = zsplit ? NI / 2 : NI;
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // (through a shuffle: the compiler then knows it is warp-uniform)
-  const int j = tid >> 3, px = tid & 7, i0 = 2 * px;
+  // thread -> (row j, pair px).  8 lanes are one row.  fp32: the two rows of a half-warp are 4 apart, so that their 64-byte
+  // segments of the primitive plane (pitch 20) and of the y array (pitch 20) fall into disjoint banks: 80 B x 4 = 320 B = 64 mod 128
+  // (with adjacent rows every 8-byte vector access of a half-warp was a 2-way bank conflict)
+  const int j = S::ROWS4 ? ((lane >> 3) << 2) + warp : tid >> 3, px = tid & 7, i0 = 2 * px;
   const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
   const T th2 = T(2) * P.theta;
   int hits = 0;
@@ -300,7 +286,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
   const T *raw = sm + S::O_RAW + j * NI + i0;                 // this pair in ring slot 0, v = 0
   T *wme = sm + S::O_W + (j + NG) * PW + (i0 + NG);           // this pair in primitive buffer 0, v = 0
   T *qx = sm + S::O_QX + j + (px == 7 ? NI : 0);              // px = 0: q+ of cell -1 of this row; px = 7: q+ of cell 15 / flux through face 16
-  T *qy = sm + S::O_QY + j * NI + i0;                         // slot j: q+ of row j-1 / flux through face j
+  T *qy = sm + S::O_QY + j * S::PY + i0;                      // slot j: q+ of row j-1 / flux through face j
 
   T Uh[NV];                                                   // halo cell of the next plane to convert
   auto halo_load = [&](int pk_) {
@@ -399,7 +385,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
         const T qpy0 = fma(qs, mr, a0);
         mr = pk::slope_mr(a1 - wd.y, wu.y - a1, wu.y - wd.y, th2, qs);
         qmy1[v] = fma(-qs, mr, a1);
-        pk::st2(qy + v * QYV + NI, qpy0, fma(qs, mr, a1));
+        pk::st2(qy + v * QYV + S::PY, qpy0, fma(qs, mr, a1));
       }
       if (warp == (c & 3)) pk::halo_slopes<T, NV, 0, S>(sm, c & 1, lane, th2);
       if (warp == ((c + 1) & 3)) pk::halo_slopes<T, NV, 1, S>(sm, c & 1, lane, th2);
@@ -525,7 +511,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
     for (int v = 0; v < NV; ++v) {
       T fxh = pk::shfl_down8(Gx0[v]);               // flux through face i0+2 = the right neighbour's low face
       if (px == 7) fxh = qx[v * QXV];               // face 16 (halo_flux)
-      const auto fyh = pk::ld2(qy + v * QYV + NI);
+      const auto fyh = pk::ld2(qy + v * QYV + S::PY);
       acc[0][v] = ((Gx1[v] - Gx0[v]) + (fyh.x - Gy0[v])) - acc[0][v];
       acc[1][v] = ((fxh - Gx1[v]) + (fyh.y - Gy1[v])) - acc[1][v];
     }
