@@ -88,3 +88,24 @@ def test_config2_kelvin_helmholtz_256_sampled_10_steps(gpu, dtype, tol):
 def test_config4_mhd_128_sampled_10_steps(gpu):
     G = wl.mhd_turbulence_global(128, gamma=5.0 / 3.0, seed=20004)
     check_fullsize(gpu, G, 5.0 / 3.0, 8, "f64", nsample=2, seed=4, tol=1e-12, steps=10, label="cfg4 128^3 10 steps")
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_large_run_is_bitwise_reproducible(gpu, dtype):
+    """A timing-dependent hazard in the stage kernel (its CTA barriers are split mbarrier halves, its rings are refilled by
+    TMA while other warps still compute) would show as run-to-run differences once thousands of CTAs compete for the SMs:
+    config 5 at 256^3 (4096 patches, 14 waves), 12 steps, twice, on two pools -- every bit of the state and every dt equal."""
+    G = wl.stress_global(256, seed=20005)
+    h = wl.uniform_hierarchy(16, periodic=True)
+    U = wl.split_global(h, G).astype(np.float64 if dtype == "f64" else np.float32)
+    del G
+    runs = []
+    for rep in range(2):
+        g = gpu.AmrHydro(h, 1.4, 5, dtype=dtype)
+        g.upload(0, U)
+        dts = [g.advance(0.3) for _ in range(12)]
+        runs.append((dts, g.download(0)))
+        del g
+    assert runs[0][0] == runs[1][0]
+    assert np.isfinite(runs[0][1]).all() and np.array_equal(runs[0][1], runs[1][1])
+    assert not np.array_equal(runs[0][1], U)
