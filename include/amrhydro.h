@@ -252,6 +252,45 @@ int amrhydro_advance_host(amrhydro_t *h, double cfl, double dt_fixed, int nsteps
 
 int amrhydro_sync(amrhydro_t *h);
 
+/* ---- a1 without any allocation -------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it): the CFL reduction of amrhydro_cfl_dt (S2-S4, the same per-cell formula) with no handle, no pool binding and NO
+ * allocation of any kind -- no cudaMalloc / cudaFree / allocating library routine is called, by set-up or by the call.
+ * The scratch of the reduction (one partial maximum per patch and a ticket counter) lives in a file-scope
+ * `static __device__` array of 256 + 8 * AMRHYDRO_NOALLOC_MAX_PATCHES bytes = 256.25 KiB, which every GPU that loads
+ * the library holds until the process exits.
+ *
+ *   dev_patches  device pointer: `npatches` consecutive patches in the pool's padded layout (what amrhydro_bind_pool
+ *                lays out: the address of patch p of slot s is pool + (s * max_patches + p) * amrhydro_pool_bytes(h,1,1)),
+ *                elements of `dtype_bits` (32 or 64) bits, `nvars` = 5, 8 or 9.  Read only; interiors are read,
+ *                ghosts are not.
+ *   gamma, rho_floor, e_floor, glm_ch   as amrhydro_create / AMRHYDRO_OPT_RHO_FLOOR / _EINT_FLOOR / _GLM_CH.
+ *   cfl_dx       cfl * dx of the level.
+ *   stream       cudaStream_t of the launch (0 = the legacy default stream).  Nothing is synchronised.
+ *   dev_out      device pointer, three doubles, written by the call: [0] the maximum signal speed over all interior
+ *                cells (+inf if any conserved value is NaN or inf), [1] dt = cfl_dx / [0], [2] 1 if [0] is zero, NaN
+ *                or inf (what amrhydro_cfl_dt reports as AMRHYDRO_ENONFINITE), else 0.
+ *
+ * Returns 0, AMRHYDRO_EINVAL (null pointer, nvars / dtype_bits / gamma / floors out of range, npatches < 1),
+ * AMRHYDRO_ENOMEM if npatches > AMRHYDRO_NOALLOC_MAX_PATCHES (the scratch array is not grown: split the level or use
+ * amrhydro_cfl_dt), AMRHYDRO_ECUDA; amrhydro_noalloc_last_error() then returns the text (per thread, static storage).
+ * Floor hits are not counted.
+ *
+ * ALL calls on one device share the one scratch array, and it keeps the last call's contents: each call clears the
+ * ticket counter on `stream` before its launch and overwrites the partial maxima it reads.  Two calls that OVERLAP on
+ * the GPU (different streams without an ordering between them, or two host threads on two streams) race on it and
+ * return garbage; calls on one stream, or ordered by events, are safe.
+ *
+ * amrhydro_noalloc_setup(): looks up the device address of the scratch array for the CURRENT device
+ * (cudaGetSymbolAddress, once per device) -- call it once per device outside any stream capture;
+ * amrhydro_cfl_dt_noalloc calls it itself when that has not happened yet.  Devices 0..63. */
+#define AMRHYDRO_NOALLOC_MAX_PATCHES 32768   /* 512^3 cells in 16^3 patches: BASELINE config 5 */
+int amrhydro_noalloc_setup(void);
+int amrhydro_cfl_dt_noalloc(const void *dev_patches, int npatches, int nvars, int dtype_bits, double gamma,
+                            double rho_floor, double e_floor, double glm_ch, double cfl_dx, void *stream,
+                            double *dev_out);
+const char *amrhydro_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

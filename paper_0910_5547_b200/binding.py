@@ -24,7 +24,9 @@ EXPORTS = [
     "amrhydro_reflux", "amrhydro_copy_slot", "amrhydro_glm_damp", "amrhydro_refine_indicator",
     "amrhydro_prolong_interior", "amrhydro_regrid", "amrhydro_set_owned", "amrhydro_set_halo_plan",
     "amrhydro_halo_bytes", "amrhydro_halo_pack", "amrhydro_halo_unpack", "amrhydro_advance", "amrhydro_advance_host", "amrhydro_sync",
+    "amrhydro_noalloc_setup", "amrhydro_cfl_dt_noalloc", "amrhydro_noalloc_last_error",
 ]
+NOALLOC_MAX_PATCHES = 32768          # AMRHYDRO_NOALLOC_MAX_PATCHES
 
 
 class PatchDesc(C.Structure):
@@ -80,12 +82,37 @@ def load_library():
     L.amrhydro_advance.argtypes = [vp, d, d, dp]
     L.amrhydro_advance_host.argtypes = [vp, d, d, i, vp, vp, dp]
     L.amrhydro_sync.argtypes = [vp]
+    L.amrhydro_noalloc_setup.argtypes = []
+    L.amrhydro_cfl_dt_noalloc.argtypes = [vp, i, i, i, d, d, d, d, d, vp, vp]
+    L.amrhydro_noalloc_last_error.restype = C.c_char_p
+    L.amrhydro_noalloc_last_error.argtypes = []
     _lib = L
     return L
 
 
 class AmrHydroError(RuntimeError):
     pass
+
+
+def _ok_noalloc(L, r):
+    if r != 0:
+        raise AmrHydroError("amrhydro error %d: %s" % (r, L.amrhydro_noalloc_last_error().decode()))
+
+
+def noalloc_setup():
+    """amrhydro_noalloc_setup: once per device, with that device current, outside stream capture."""
+    L = load_library()
+    _ok_noalloc(L, L.amrhydro_noalloc_setup())
+
+
+def cfl_dt_noalloc(dev_patches, npatches, nvars, dtype_bits, gamma, cfl_dx, dev_out, stream=0,
+                   rho_floor=1e-30, e_floor=1e-30, ch=1.0):
+    """amrhydro_cfl_dt_noalloc: the CFL reduction over `npatches` consecutive patches at device address `dev_patches`
+    (pool layout) with its scratch in a static device array -- no handle, no allocation.  dev_out: device address of
+    three doubles (max signal speed, dt = cfl_dx / max, non-finite flag).  Nothing is synchronised."""
+    L = load_library()
+    _ok_noalloc(L, L.amrhydro_cfl_dt_noalloc(dev_patches, int(npatches), int(nvars), int(dtype_bits), float(gamma),
+                                             float(rho_floor), float(e_floor), float(ch), float(cfl_dx), stream, dev_out))
 
 
 class AmrHydro:
@@ -180,6 +207,12 @@ class AmrHydro:
             self.close()
         except Exception:
             pass
+
+    def patch_ptr(self, slot, patch):
+        """Device address of 16^3 patch `patch` of `slot` in the pool (the layout amrhydro_cfl_dt_noalloc reads)."""
+        if self.pdim != 16:
+            raise AmrHydroError("patch_ptr is defined for 16^3 patches")
+        return self.pool.data_ptr() + (slot * self.max_patches + patch) * int(self.L.amrhydro_pool_bytes(self.h, 1, 1))
 
     # ---- options / counters
     def set_option(self, key, value):

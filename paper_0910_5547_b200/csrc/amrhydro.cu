@@ -1237,3 +1237,178 @@ int amrhydro_sync(amrhydro_t *h) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// a1 without any allocation (include/amrhydro.h: amrhydro_cfl_dt_noalloc).  A variant of k_cfl whose scratch -- one
+// partial maximum per patch and a ticket counter -- is a file-scope __device__ array instead of handle-owned memory:
+// block b publishes the bits of its maximum in words 32 + b, takes a ticket, and the block that draws the last ticket
+// reduces the partial maxima (max is exact in any order) and writes the three output doubles.
+//
+// g_noalloc_scratch names DEVICE memory.  In host code the identifier is only a host-side stand-in: its device address
+// comes from cudaGetSymbolAddress, once per device with that device current (noalloc_scratch_ptr), and that pointer is
+// what the kernel is given.  Word 0: ticket counter (must be zero when a launch starts: cleared by a memset node on the
+// launch stream before every launch, and reset by the last block).  Words 1..31: padding to 256 bytes.
+#include <cstdarg>
+#include <mutex>
+
+namespace {
+
+constexpr int NOALLOC_HDR = 32;                                             // 64-bit words before the partial maxima
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static __device__ __align__(256) unsigned long long g_noalloc_scratch[NOALLOC_HDR + AMRHYDRO_NOALLOC_MAX_PATCHES];
+
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_cfl_noalloc(const T *__restrict__ patches, Params<T> P, double cfl_dx,
+                                                     unsigned long long *__restrict__ scratch, double *__restrict__ out) {
+  const T *Ub = patches + size_t(blockIdx.x) * size_t(NV) * Layout<T>::VS;
+  const int i = threadIdx.x & 15, j = threadIdx.x >> 4;
+  T best = T(0);
+  int hits = 0;
+  bool bad = false;
+#pragma unroll 4
+  for (int k = 0; k < NI; ++k) {                    // the per-cell arithmetic of k_cfl (kernels_level.cuh), S2-S4
+    T U[NV], W[NV];
+    const int c = cell<T>(k + NG, j + NG, i + NG);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) U[v] = Ub[size_t(v) * Layout<T>::VS + c];
+    cons_to_prim<T, NV>(U, W, P, hits);
+    T s = max_signal_speed<T, NV>(W, P);
+    T chk = s;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) chk += U[v];
+    bad |= !(chk - chk == T(0));                   // NaN or inf anywhere
+    best = tmax(best, s);
+  }
+  double b = bad ? __longlong_as_double(0x7ff0000000000000LL) : double(best);
+  __shared__ double wmax[8];
+  __shared__ bool last;
+  auto block_max = [&](double x) {                  // result valid in thread 0
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      x = threadIdx.x < 8 ? wmax[threadIdx.x] : 0.0;
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+    }
+    return x;
+  };
+  b = block_max(b);
+  if (threadIdx.x == 0) {
+    __stcg(scratch + NOALLOC_HDR + blockIdx.x, (unsigned long long)__double_as_longlong(b));
+    __threadfence();                                // the partial maximum is visible before the ticket is
+    last = atomicAdd(scratch, 1ULL) == (unsigned long long)(gridDim.x - 1);
+  }
+  __syncthreads();                                  // also orders the reads of wmax above before the writes below
+  if (!last) return;
+  __threadfence();
+  double m = 0.0;                                   // non-negative doubles or +inf, never NaN
+  for (int q = threadIdx.x; q < (int)gridDim.x; q += 256)
+    m = fmax(m, __longlong_as_double((long long)__ldcg(scratch + NOALLOC_HDR + q)));
+  m = block_max(m);
+  if (threadIdx.x == 0) {
+    out[0] = m;
+    out[1] = cfl_dx / m;
+    out[2] = (m > 0.0 && m < __longlong_as_double(0x7ff0000000000000LL)) ? 0.0 : 1.0;
+    scratch[0] = 0ULL;                              // leave the ticket at zero for the next call
+  }
+}
+
+std::mutex g_noalloc_mu;
+unsigned long long *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};                // device address of the array, per device
+thread_local char g_noalloc_err[320] = "";
+
+int noalloc_fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_noalloc_err, sizeof(g_noalloc_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+// the device address of g_noalloc_scratch on the current device (looked up once per device)
+int noalloc_scratch_ptr(unsigned long long **ptr) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return noalloc_fail(AMRHYDRO_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES)
+    return noalloc_fail(AMRHYDRO_EINVAL, "device %d is outside 0..%d", dev, NOALLOC_MAX_DEVICES - 1);
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p)
+      return noalloc_fail(AMRHYDRO_ECUDA, "cudaGetSymbolAddress(g_noalloc_scratch) on device %d: %s", dev,
+                          cudaGetErrorString(e));
+    g_noalloc_ptr[dev] = static_cast<unsigned long long *>(p);
+  }
+  *ptr = g_noalloc_ptr[dev];
+  return 0;
+}
+
+template <typename T, int NV>
+int launch_cfl_noalloc(const void *patches, int np, double gamma, double rho_floor, double e_floor, double ch, double cfl_dx,
+                       cudaStream_t st, unsigned long long *scratch, double *out) {
+  Params<T> P;
+  P.gamma = T(gamma);
+  P.gm1 = T(gamma - 1.0);
+  P.gg1 = T(gamma * (gamma - 1.0));
+  P.theta = T(1.5);                                 // not read by the reduction
+  P.rho_floor = T(rho_floor);
+  P.e_floor = T(e_floor);
+  P.ch = T(ch);
+  k_cfl_noalloc<T, NV><<<np, 256, 0, st>>>(static_cast<const T *>(patches), P, cfl_dx, scratch, out);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return noalloc_fail(AMRHYDRO_ECUDA, "launch of k_cfl_noalloc: %s", cudaGetErrorString(e));
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int amrhydro_noalloc_setup(void) {
+  unsigned long long *p = nullptr;
+  return noalloc_scratch_ptr(&p);
+}
+
+const char *amrhydro_noalloc_last_error(void) { return g_noalloc_err; }
+
+int amrhydro_cfl_dt_noalloc(const void *dev_patches, int npatches, int nvars, int dtype_bits, double gamma,
+                            double rho_floor, double e_floor, double glm_ch, double cfl_dx, void *stream, double *dev_out) {
+  if (!dev_patches || !dev_out) return noalloc_fail(AMRHYDRO_EINVAL, "dev_patches / dev_out is null");
+  if (nvars != 5 && nvars != 8 && nvars != 9) return noalloc_fail(AMRHYDRO_EINVAL, "nvars must be 5, 8 or 9 (got %d)", nvars);
+  if (dtype_bits != 32 && dtype_bits != 64) return noalloc_fail(AMRHYDRO_EINVAL, "dtype_bits must be 32 or 64 (got %d)", dtype_bits);
+  if (!(gamma > 1.0) || !std::isfinite(gamma)) return noalloc_fail(AMRHYDRO_EINVAL, "gamma must be > 1 and finite");
+  if (!(rho_floor > 0.0) || !std::isfinite(rho_floor) || !(e_floor > 0.0) || !std::isfinite(e_floor))
+    return noalloc_fail(AMRHYDRO_EINVAL, "floors must be positive and finite");
+  if (nvars == 9 && (!(glm_ch > 0.0) || !std::isfinite(glm_ch))) return noalloc_fail(AMRHYDRO_EINVAL, "c_h must be positive and finite");
+  if (!std::isfinite(cfl_dx)) return noalloc_fail(AMRHYDRO_EINVAL, "cfl_dx must be finite");
+  if (npatches < 1) return noalloc_fail(AMRHYDRO_EINVAL, "npatches must be >= 1 (got %d)", npatches);
+  if (npatches > AMRHYDRO_NOALLOC_MAX_PATCHES)
+    return noalloc_fail(AMRHYDRO_ENOMEM, "npatches = %d exceeds AMRHYDRO_NOALLOC_MAX_PATCHES = %d: the static scratch array holds "
+                        "one partial maximum per patch and is not grown (split the level or use amrhydro_cfl_dt)",
+                        npatches, AMRHYDRO_NOALLOC_MAX_PATCHES);
+  if ((uintptr_t)dev_patches % (dtype_bits / 8) || (uintptr_t)dev_out % 8)
+    return noalloc_fail(AMRHYDRO_EINVAL, "dev_patches / dev_out is not aligned to its element size");
+  unsigned long long *scratch = nullptr;
+  if (int r = noalloc_scratch_ptr(&scratch)) return r;
+  cudaStream_t st = (cudaStream_t)stream;
+  // the ticket counter must start at zero whatever an earlier (possibly failed) launch left behind
+  cudaError_t e = cudaMemsetAsync(scratch, 0, NOALLOC_HDR * sizeof(unsigned long long), st);
+  if (e != cudaSuccess) return noalloc_fail(AMRHYDRO_ECUDA, "cudaMemsetAsync(scratch header): %s", cudaGetErrorString(e));
+#define NOALLOC_CASE(T, NV)                                                                                              \
+  return launch_cfl_noalloc<T, NV>(dev_patches, npatches, gamma, rho_floor, e_floor, glm_ch, cfl_dx, st, scratch, dev_out)
+  if (dtype_bits == 64) {
+    if (nvars == 5) NOALLOC_CASE(double, 5);
+    if (nvars == 8) NOALLOC_CASE(double, 8);
+    NOALLOC_CASE(double, 9);
+  }
+  if (nvars == 5) NOALLOC_CASE(float, 5);
+  if (nvars == 8) NOALLOC_CASE(float, 8);
+  NOALLOC_CASE(float, 9);
+#undef NOALLOC_CASE
+}
+
+}  // extern "C"
