@@ -51,8 +51,8 @@ struct amrhydro {
   Desc *d_desc = nullptr;
   int *d_child = nullptr, *d_octant = nullptr;
   void *d_Rf = nullptr, *d_Rc = nullptr, *d_bflux = nullptr;
-  // found once per hierarchy, so that the per-level launches carry no idle blocks: patches with a coarse-fine region
-  // (k_fill_ghosts when sibling copies are skipped), flux-register tasks (local patch * 64 + task of k_flux_registers),
+  // found once per hierarchy, so that the per-level launches carry no idle blocks: coarse-fine faces (patch * 8 + face:
+  // the tasks of k_fill_cf_faces when sibling copies are skipped), flux-register tasks (local patch * 64 + task of k_flux_registers),
   // and per patch the boundary-flux planes a register reads (bit 3 d + s; rk_stage stores only those)
   int *d_cflist = nullptr, *d_frtasks = nullptr, *d_bneed = nullptr;
   std::vector<int> cf_first, cf_count, fr_first, fr_count;
@@ -453,12 +453,10 @@ static int install_hierarchy(amrhydro_t *h, const amrhydro_patch_desc *tbl, int 
       h->cf_first[l] = int(cfl.size());
       h->fr_first[l] = int(frt.size());
       for (int p = first[l]; p < first[l] + count[l]; ++p) {
-        bool cf = false;
-        for (int r = 0; r < 27; ++r) cf |= (r != 13 && tbl[p].nbr[r] == -1);
-        if (cf) cfl.push_back(p);
         const int pl = p - first[l];
         for (int f = 0; f < 6; ++f)                           // fine side of a coarse-fine face
           if (l > 0 && tbl[p].nbr[face_region(f)] == -1) {
+            cfl.push_back(p * 8 + f);
             frt.push_back(pl * 64 + f);
             bneed[p] |= 1 << ((f >> 1) * 3 + ((f & 1) ? 2 : 0));
           }
@@ -773,12 +771,16 @@ static int fill_ghosts_impl(amrhydro_t *h, int level, int slot, int pold, int pn
   return dispatch(h, [&](auto t, auto nv) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
-    if (phase1) {
-      // sibling copies skipped: only the patches with a coarse-fine region have anything to fill
-      const int nb = skip ? h->cf_count[level] : h->lev_run[level];
-      k_fill_ghosts<T, NV><<<dim3(nb, NP), 256, 0, h->stream>>>(
-          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, skip,
-          skip ? h->d_cflist + h->cf_first[level] : nullptr);
+    if (phase1 && skip) {
+      // sibling copies skipped: all there is to fill is the slab behind every coarse-fine face of the level
+      if (h->cf_count[level] > 0) {
+        k_fill_cf_faces<T, NV><<<h->cf_count[level], 256, 0, h->stream>>>(
+            make_pool<T>(h), slot, pold, pnew, T(alpha), h->d_desc, h->d_octant, h->d_cflist + h->cf_first[level]);
+        LAUNCH_CHECK(h);
+      }
+    } else if (phase1) {
+      k_fill_ghosts<T, NV><<<dim3(h->lev_run[level], NP), 256, 0, h->stream>>>(
+          make_pool<T>(h), slot, pold, pnew, T(alpha), h->lev_first[level], h->d_desc, h->d_octant, 0);
       LAUNCH_CHECK(h);
     }
     if (phase2) {
@@ -798,7 +800,7 @@ static int materialise_sibling_ghosts(amrhydro_t *h, int level, int slot) {
     using T = decltype(t);
     constexpr int NV = decltype(nv)::value;
     k_fill_ghosts<T, NV><<<dim3(h->lev_run[level], NP), 256, 0, h->stream>>>(
-        make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2, nullptr);
+        make_pool<T>(h), slot, slot, slot, T(0), h->lev_first[level], h->d_desc, h->d_octant, 2);
     LAUNCH_CHECK(h);
     return 0;
   });

@@ -144,24 +144,22 @@ template <typename T> __device__ __forceinline__ T minmod2(T a, T b) {
 // copied from that sibling's interior; where it is a coarse-fine boundary it is prolongated
 // from the parent's padded box, conservative limited-linear (S6) in time-interpolated parent
 // data (S7; alpha = 0 or 1 reads only the slot that counts, which is the same value bitwise for
-// finite data).  mode bit 0: sibling face/edge/corner copies are skipped (rk_stage reads siblings directly);
-// bit 1: the prolongation is skipped (siblings only: refine_indicator / download_padded in direct-halo mode).
+// finite data).  mode bit 1: the prolongation is skipped (siblings only: refine_indicator / download_padded in
+// direct-halo mode).  Where only rk_stage will read the ghosts and it reads siblings directly (direct halos on the
+// finest level, the fill of U1 on any level), k_fill_cf_faces below does the work instead.
 // Phase 2 (k_fill_outflow, launched only for levels that touch an outflow boundary): zero-gradient
 // outflow, x then y then z over the full padded extent, one block per patch.
 template <typename T, int NV>
 __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int pold, int pnew, T alpha,
                                                      int first, const Desc *__restrict__ desc,
-                                                     const int *__restrict__ octant, int mode,
-                                                     const int *__restrict__ plist) {
+                                                     const int *__restrict__ octant, int mode) {
   // Latency is what this kernel costs on small AMR levels, so it is written as two dependent round trips to
   // memory: (1) the patch's descriptor row and octant (every thread reads what it needs, broadcast through
   // L1: no staging, no barrier), (2) all parent cells this plane prolongates from -- 3 coarse planes x 12 x 12
   // per variable, time-interpolated once (S7) into shared memory -- together with the sibling cells to copy.
   // A fine patch is an octant of its parent and origins are multiples of 16, so parent indices follow from
   // the octant bits alone: coarse index of padded fine index t along d = 8 oc_d + floor((t - 2) / 2) + 2.
-  // plist (may be null): the patches of the level that have a coarse-fine region (all this launch has to fill when
-  // the sibling copies are skipped), so that a level of thousands of interior patches launches no idle blocks
-  const int p = plist ? plist[blockIdx.x] : first + blockIdx.x, k = blockIdx.y;
+  const int p = first + blockIdx.x, k = blockIdx.y;
   const Desc &D = desc[p];
   T *U = pool.patch(slot, p);
   constexpr int CT = 12, CTV = 3 * CT * CT;
@@ -170,20 +168,9 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
   const int oz = k < NG ? -1 : (k >= NG + NI ? 1 : 0);
   const int *nbr = D.nbr + (oz + 1) * 9;             // the nine regions of this plane
   bool cf = false;                                   // block-uniform: does this plane touch a coarse-fine region?
-  const bool skip_siblings = mode & 1;
-  // faces_only (sibling copies skipped = direct halos on the finest level): only the six face slabs are read by anyone
-  // (rk_stage), so edge and corner regions are left alone and the parent tile is loaded only where a
-  // face slab prolongates from it
-  const bool faces_only = skip_siblings;
-  bool fxl = false, fxh = false, fyl = false, fyh = false;
   if (Q >= 0 && !(mode & 2)) {
-    if (faces_only) {
-      if (oz != 0) cf = nbr[4] == -1;
-      else { fxl = nbr[3] == -1; fxh = nbr[5] == -1; fyl = nbr[1] == -1; fyh = nbr[7] == -1; cf = fxl | fxh | fyl | fyh; }
-    } else {
 #pragma unroll
-      for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
-    }
+    for (int r = 0; r < 9; ++r) cf |= ((oz + 1) * 9 + r != 13) && nbr[r] == -1;
   }
   int pc0[3] = {0, 0, 0};                            // parent padded index of the tile's first cell
   if (cf) {
@@ -195,18 +182,12 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
     const bool only_old = alpha == T(0), only_new = alpha == T(1);
     // 432 tile cells per variable over 256 threads: two cells per thread, their parent offsets computed once
     const int r0 = threadIdx.x, r1 = threadIdx.x + 256;
-    // (faces_only, interior plane: a tile cell is needed if it lies within the three coarse columns / rows of a face slab)
-    auto needed = [&](int r) {
-      if (!faces_only || oz != 0) return true;
-      const int tx = r % CT, ty = (r / CT) % CT;
-      return (fxl && tx <= 2) || (fxh && tx >= CT - 3) || (fyl && ty <= 2) || (fyh && ty >= CT - 3);
-    };
-    const int c0 = needed(r0) ? cell<T>(pc0[2] + r0 / (CT * CT), pc0[1] + (r0 / CT) % CT, pc0[0] + r0 % CT) : -1;
-    const int c1 = r1 < CTV && needed(r1) ? cell<T>(pc0[2] + r1 / (CT * CT), pc0[1] + (r1 / CT) % CT, pc0[0] + r1 % CT) : -1;
+    const int c0 = cell<T>(pc0[2] + r0 / (CT * CT), pc0[1] + (r0 / CT) % CT, pc0[0] + r0 % CT);
+    const int c1 = r1 < CTV ? cell<T>(pc0[2] + r1 / (CT * CT), pc0[1] + (r1 / CT) % CT, pc0[0] + r1 % CT) : -1;
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const T *po = Co + size_t(v) * Layout<T>::VS, *pn = Cn + size_t(v) * Layout<T>::VS;
-      if (c0 >= 0) s_par[v * CTV + r0] = only_old ? po[c0] : (only_new ? pn[c0] : (T(1) - alpha) * po[c0] + alpha * pn[c0]);
+      s_par[v * CTV + r0] = only_old ? po[c0] : (only_new ? pn[c0] : (T(1) - alpha) * po[c0] + alpha * pn[c0]);
       if (c1 >= 0) s_par[v * CTV + r1] = only_old ? po[c1] : (only_new ? pn[c1] : (T(1) - alpha) * po[c1] + alpha * pn[c1]);
     }
   }
@@ -218,18 +199,16 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
     else { const int u = t - 2 * NG * NP; j = NG + u / (2 * NG); i = u % (2 * NG); if (i >= NG) i += NI; }
   };
   // sibling copies first: their loads travel with the tile's
-  if (!skip_siblings) {
-    for (int t = threadIdx.x; t < ncell; t += 256) {
-      int i, j;
-      locate(t, i, j);
-      const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
-      const int nb = nbr[(oy + 1) * 3 + (ox + 1)];
-      if (nb < 0) continue;
-      const T *S = pool.patch(slot, nb);
-      const int me = cell<T>(k, j, i), sc = cell<T>(k - oz * NI, j - oy * NI, i - ox * NI);
+  for (int t = threadIdx.x; t < ncell; t += 256) {
+    int i, j;
+    locate(t, i, j);
+    const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
+    const int nb = nbr[(oy + 1) * 3 + (ox + 1)];
+    if (nb < 0) continue;
+    const T *S = pool.patch(slot, nb);
+    const int me = cell<T>(k, j, i), sc = cell<T>(k - oz * NI, j - oy * NI, i - ox * NI);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + me] = S[size_t(v) * Layout<T>::VS + sc];
-    }
+    for (int v = 0; v < NV; ++v) U[size_t(v) * Layout<T>::VS + me] = S[size_t(v) * Layout<T>::VS + sc];
   }
   if (!cf) return;                                   // block-uniform
   __syncthreads();
@@ -238,7 +217,6 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
     locate(t, i, j);
     const int ox = i < NG ? -1 : (i >= NG + NI ? 1 : 0), oy = j < NG ? -1 : (j >= NG + NI ? 1 : 0);
     if (nbr[(oy + 1) * 3 + (ox + 1)] != -1) continue;
-    if (faces_only && (ox != 0) + (oy != 0) + (oz != 0) != 1) continue;      // edge / corner region: nobody reads it
     const int pad[3] = {i, j, k};
     int c0 = 0;
     T s[3];
@@ -259,6 +237,73 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(Pool<T> pool, int slot, int
       T val = uc;
 #pragma unroll
       for (int d = 0; d < 3; ++d) val = val + s[d] * minmod2(c[c0 + st[d]] - uc, uc - c[c0 - st[d]]);
+      U[size_t(v) * Layout<T>::VS + me] = val;
+    }
+  }
+}
+
+// The same prolongation (S6, S7: the expressions of k_fill_ghosts, term by term) for the fills whose only reader is
+// rk_stage with direct sibling halos: nobody reads sibling ghosts, edge or corner regions then (the stage
+// needs the two layers behind each FACE), so all there is to fill is the 2 x 16 x 16 slab behind every coarse-fine
+// face.  One block per (patch, face) task = patch * 8 + face: the slab prolongates from 3 x 10 x 10 parent cells per
+// variable (one coarse layer + its two neighbours for the slope, 8 + 2 cells along each tangential direction), staged
+// once in shared memory, two fine cells per thread.  A level of thousands of patches launches one block per face
+// instead of twenty per patch, and each parent cell is read once instead of up to ten times.
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) k_fill_cf_faces(Pool<T> pool, int slot, int pold, int pnew, T alpha,
+                                                       const Desc *__restrict__ desc, const int *__restrict__ octant,
+                                                       const int *__restrict__ tasks) {
+  const int task = tasks[blockIdx.x], p = task >> 3, f = task & 7, d = f >> 1, side = f & 1;
+  const int Q = desc[p].parent, o = octant[p];
+  const int e1 = d == 0 ? 1 : 0, e2 = d == 2 ? 1 : 2;          // the tangential dimensions, ascending
+  constexpr int CT = 10, CTV = 3 * CT * CT;
+  __shared__ T s_par[NV * CTV];
+  int pc0[3], st[3];                                           // parent padded index of the tile's first cell; tile strides
+  pc0[d] = 8 * ((o >> d) & 1) + (side ? 8 : -1) + NG - 1;      // the coarse layer behind the face is fc = -1 or 8
+  pc0[e1] = 8 * ((o >> e1) & 1) + NG - 1;
+  pc0[e2] = 8 * ((o >> e2) & 1) + NG - 1;
+  st[d] = CT * CT; st[e1] = 1; st[e2] = CT;
+  {
+    const T *Co = pool.patch(pold, Q), *Cn = pool.patch(pnew, Q);
+    const bool only_old = alpha == T(0), only_new = alpha == T(1);
+    for (int r = threadIdx.x; r < CTV; r += 256) {
+      int pc[3];
+      pc[d] = pc0[d] + r / (CT * CT); pc[e1] = pc0[e1] + r % CT; pc[e2] = pc0[e2] + (r / CT) % CT;
+      const int c = cell<T>(pc[2], pc[1], pc[0]);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const T *po = Co + size_t(v) * Layout<T>::VS, *pn = Cn + size_t(v) * Layout<T>::VS;
+        s_par[v * CTV + r] = only_old ? po[c] : (only_new ? pn[c] : (T(1) - alpha) * po[c] + alpha * pn[c]);
+      }
+    }
+  }
+  __syncthreads();
+  T *U = pool.patch(slot, p);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int t = threadIdx.x + 256 * h;                       // 512 ghost cells; x fastest among the threads of a warp
+    int g, a, b;
+    if (d == 0) { g = t & 1; a = (t >> 1) & 15; b = t >> 5; }
+    else { a = t & 15; b = (t >> 4) & 15; g = t >> 8; }
+    int pad[3];
+    pad[d] = side ? NG + NI + g : g; pad[e1] = NG + a; pad[e2] = NG + b;
+    int c0 = 0;
+    T s[3];
+#pragma unroll
+    for (int dd = 0; dd < 3; ++dd) {
+      const int fr = pad[dd] - NG;                   // fine index relative to the patch (>= -2)
+      const int fc = (fr + 64) / 2 - 32;             // floor(fr/2)
+      s[dd] = (fr - 2 * fc == 0) ? T(-0.25) : T(0.25);
+      c0 += (8 * ((o >> dd) & 1) + fc + NG - pc0[dd]) * st[dd];
+    }
+    const int me = cell<T>(pad[2], pad[1], pad[0]);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const T *c = s_par + v * CTV;
+      const T uc = c[c0];
+      T val = uc;
+#pragma unroll
+      for (int dd = 0; dd < 3; ++dd) val = val + s[dd] * minmod2(c[c0 + st[dd]] - uc, uc - c[c0 - st[dd]]);
       U[size_t(v) * Layout<T>::VS + me] = val;
     }
   }
