@@ -285,14 +285,16 @@ template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18, 
 #define AMR_BASE_TMA 1      // combination stage: U_base planes come through their own TMA ring (no global loads in the warps)
 #endif
 template <typename T, int NV, bool WB = true> struct Smem {   // WB: the kernel reads U_base (combination stage)
-  static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY, NSLOT = Cfg<T>::NSLOT;
+  static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY;
+  // (the fp64 GLM-9 combination stage takes a ring of three, the minimum, so that its U_base ring fits beside it)
+  static constexpr int NSLOT = (WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 9) ? 3 : Cfg<T>::NSLOT;
   static constexpr int RAWP = NV * NI * NI;        // one raw plane: [NV][16][16], dense TMA box
   static constexpr int WV = NP * PW;               // one variable of one primitive plane [20][PW]
   static constexpr int QXV = NI * PQ;              // [16][PQ]: slot s = q+ of cell s-1 / flux at face s
   static constexpr int QYV = (NI + 1) * PY;        // [17][PY]
   // the flux arrays alias the q+ arrays (slot s is read as q+ by its only reader before that same thread overwrites it
   // with the flux) in the fp64 MHD combination stage, so that its U_base ring fits
-  static constexpr bool ALIAS = WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 8;
+  static constexpr bool ALIAS = WB && AMR_BASE_TMA && sizeof(T) == 8 && NV >= 8;
   static constexpr int O_RAW = 0, O_W = O_RAW + NSLOT * RAWP, O_QX = O_W + 2 * NV * WV,
                        O_FX = ALIAS ? O_QX : O_QX + NV * QXV, O_QY = O_FX + NV * QXV,
                        O_FY = ALIAS ? O_QY : O_QY + NV * QYV, O_ACC = O_FY + NV * QYV;
@@ -499,17 +501,15 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         for (int v = 0; v < NV; ++v) Un[v] = raw[slot * RAWP + v * (NI * NI)];
         mk::prim<T, NV>(Un, Wn, P, hits);
       }
-      if (c + 1 < NG + nz) {
+      if (c < NG + nz) {                              // (the first ghost plane above too: Wc of the last pass is re-read from here)
         T *w = wme + ((c + 1) & 1) * (NV * WV);
 #pragma unroll
         for (int v = 0; v < NV; ++v) w[v * WV] = Wn[v];
       }
       T ub[NV];
-      if (BASE && c > NG) {
+      if (BASE && !S::BTMA && c > NG) {             // (global loads: issued early; the TMA ring is read where it is used)
 #pragma unroll
-        for (int v = 0; v < NV; ++v)
-          ub[v] = S::BTMA ? raw[S::O_BRAW - S::O_RAW + ((c + 1) % S::NSLOT) * RAWP + v * (NI * NI)]   // arrived with plane c+1
-                               : base[size_t(v) * VS + (c - 1 + zlo) * PLANE];
+        for (int v = 0; v < NV; ++v) ub[v] = base[size_t(v) * VS + (c - 1 + zlo) * PLANE];
       }
       // 2. z: slope of cell c, flux through the face between c-1 and c, finish cell c-1
       T Gz[NV];
@@ -540,7 +540,8 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
           T pre = b * ui[v * (NI * NI)];
-          if (BASE) pre = fma(a, ub[v], pre);
+          if (BASE) pre = fma(a, S::BTMA ? raw[S::O_BRAW - S::O_RAW + ((c + 1) % S::NSLOT) * RAWP + v * (NI * NI)]   // arrived with plane c+1
+                                         : ub[v], pre);
           un[v] = fma(-kk, acc[v] + Gz[v], pre);                    // Eq. 7-8
           o[size_t(v) * VS] = un[v];
         }
@@ -599,8 +600,13 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         for (int v = 0; v < NV; ++v)
           acc[v] = ((fx[v * QXV + 1] - Gx[v]) + (fy[v * QYV + PY] - Gy[v])) - Gz[v];
       }
+      // W of plane c+1 comes back from the primitive buffer instead of staying in registers over the x/y phases (it is
+      // dead after the z slope, Wc after the x/y slopes: 4 NV registers less at the peak of the pass)
+      if (c < NG + nz) {
+        const T *w = wme + ((c + 1) & 1) * (NV * WV);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) Wc[v] = Wn[v];
+        for (int v = 0; v < NV; ++v) Wc[v] = w[v * WV];
+      }
     }
     if (BASE && smax_out) {
       // one atomicMax per warp on the bit pattern of a non-negative double (monotone as an unsigned integer)
