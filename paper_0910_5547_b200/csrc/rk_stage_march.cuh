@@ -460,11 +460,23 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     T *wme = sm + S::O_W + (j + NG) * PW + (i + NG);             // this column in primitive plane 0, v = 0
     T *qx = sm + S::O_QX + j * PQ + i, *fx = sm + S::O_FX + j * PQ + i;   // slot i: q+ of cell i-1 / flux at face i
     T *qy = sm + S::O_QY + j * PY + i, *fy = sm + S::O_FY + j * PY + i;
-    T Wc[NV], dzm[NV], qpz[NV], acc[NV];
+    T dzm[NV], qpz[NV], acc[NV];
     T best = T(0);                      // fused CFL reduction (a1) over the cells this thread finishes
     bool bad = false;
+    // raw plane pk -> primitives of this column in primitive buffer pk & 1
+    auto convert = [&](int pk) {
+      const int slot = pk % S::NSLOT;
+      mk::mbar_wait(&bars[slot], unsigned(pk / S::NSLOT) & 1u);
+      T Un[NV], Wn[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Un[v] = raw[slot * RAWP + v * (NI * NI)];
+      mk::prim<T, NV>(Un, Wn, P, hits);
+      T *w = wme + (pk & 1) * (NV * WV);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) w[v * WV] = Wn[v];
+    };
     {
-      T U0[NV], U1[NV], U2[NV], W0[NV], W1[NV];
+      T U0[NV], U1[NV], U2[NV], W0[NV], W1[NV], Wc[NV];
       mk::mbar_wait(&bars[0], 0);
 #pragma unroll
       for (int v = 0; v < NV; ++v) U0[v] = raw[v * (NI * NI)];
@@ -488,23 +500,19 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
       }
     }
     __syncthreads();
+    convert(NG + 1);
 
+    // The primitives of this column live in the two primitive buffers, not in registers: plane c and c+1 are read where
+    // the z slope needs them, and plane c+2 is converted at the END of pass c, when only dzm, qpz and acc are live (its
+    // buffer, that of plane c, is free once every thread is past the x/y slopes: the second barrier of the pass)
 #pragma unroll 1
     for (int c = NG; c <= NG + nz; ++c) {            // current cell = plane c of this march (2..nz+1); c = nz+2: last z face only
-      // 1. plane c+1: raw -> primitives, publish for the x/y neighbours
-      T Wn[NV];
+      const T *w = wme + (c & 1) * (NV * WV);
+      T Wc[NV], Wn[NV];
       {
-        const int slot = (c + 1) % S::NSLOT;
-        mk::mbar_wait(&bars[slot], unsigned((c + 1) / S::NSLOT) & 1u);
-        T Un[NV];
+        const T *wn = wme + ((c + 1) & 1) * (NV * WV);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Un[v] = raw[slot * RAWP + v * (NI * NI)];
-        mk::prim<T, NV>(Un, Wn, P, hits);
-      }
-      if (c < NG + nz) {                              // (the first ghost plane above too: Wc of the last pass is re-read from here)
-        T *w = wme + ((c + 1) & 1) * (NV * WV);
-#pragma unroll
-        for (int v = 0; v < NV; ++v) w[v * WV] = Wn[v];
+        for (int v = 0; v < NV; ++v) { Wc[v] = w[v * WV]; Wn[v] = wn[v * WV]; }
       }
       T ub[NV];
       if (BASE && !S::BTMA && c > NG) {             // (global loads: issued early; the TMA ring is read where it is used)
@@ -557,7 +565,6 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
       }
       if (c < NG + nz) {
         // 3. x/y phase 1: slopes of this cell along x and y, publish q+
-        const T *w = wme + (c & 1) * (NV * WV);
         T qmx[NV], qmy[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
@@ -599,13 +606,8 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
 #pragma unroll
         for (int v = 0; v < NV; ++v)
           acc[v] = ((fx[v * QXV + 1] - Gx[v]) + (fy[v * QYV + PY] - Gy[v])) - Gz[v];
-      }
-      // W of plane c+1 comes back from the primitive buffer instead of staying in registers over the x/y phases (it is
-      // dead after the z slope, Wc after the x/y slopes: 4 NV registers less at the peak of the pass)
-      if (c < NG + nz) {
-        const T *w = wme + ((c + 1) & 1) * (NV * WV);
-#pragma unroll
-        for (int v = 0; v < NV; ++v) Wc[v] = w[v * WV];
+        // 6. plane c+2: raw -> primitives, for the z slope of the next pass and the x/y neighbours of the one after
+        convert(c + 2);
       }
     }
     if (BASE && smax_out) {
