@@ -319,7 +319,7 @@ def run_ours(args):
             b1, b2 = 2 * nv * esz * cells, 3 * nv * esz * cells       # stage 1: read U write U1; stage 2: + read Un
             avg_ms = 0.5 * (s1 + s2)
             ach = 0.5 * (b1 + b2) / (avg_ms * 1e-3) / 1e9
-            key = "%s_%s" % (args.workload, dtype)
+            key = "%s_%s" % (args.workload, dtype) if not args.size else "%s_%d_%s" % (args.workload, args.size, dtype)
             traffic = NCU_TRAFFIC.get(key)
             roof = {"bound": "hbm", "kernel": {0: "k_rk_stage_ref", 2: "k_rk_stage_march", 3: "k_rk_stage_pair" if nv == 5 else "k_rk_stage_march"}[args.kernel],
                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
