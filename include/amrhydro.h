@@ -67,7 +67,11 @@ extern "C" {
 
 #define AMRHYDRO_OPT_ZSPLIT 10     /* default rk_stage kernel: two CTAs per patch, each marching over half of the column
                                      (3 warm-up planes more per CTA, about half the latency of a launch):
-                                     0 = never, 1 = always, 2 (default) = on levels of at most SMs/2 patches; any time */
+                                     0 = never, 1 = always, 2 (default) = on levels of at most SMs/2 patches, and (the
+                                     8- / 9-variable kernel) for the patches of the last wave of a launch when that wave is
+                                     less than half full (its half-CTAs all fit: 0.6 instead of 1 wave time; config 4's 512
+                                     patches are 3.46 waves of 148 CTAs: 0.490 -> 0.450 ms per step).  Bitwise the unsplit
+                                     march; any time */
 
 #define AMRHYDRO_OPT_GRAPH 11      /* amrhydro_advance replays one CUDA graph per coarse step (dt may stay in
                                      device memory for graph capture): the S9 recursion is captured once per hierarchy

@@ -60,7 +60,7 @@ struct amrhydro {
   unsigned long long *d_scalars = nullptr;  // [0] scratch, [1] floor hits
   unsigned long long *d_smax = nullptr;     // per level: bits of the max signal speed of (level, smax_slot[level])
   std::vector<int> smax_slot;               // slot the cached value belongs to, -1 = stale
-  int zsplit = 2;                           // rk_stage_march: 0 never, 1 always, 2 = levels of at most num_sms/2 patches
+  int zsplit = 2;                           // z-split of the stage kernels: 0 never, 1 always, 2 = small levels and the thin last wave of a launch
   int num_sms = 148;
   int fuse_cfl = 2;                         // 0 never, 1 / 2 = the combination stage also reduces the max signal speed
   void *d_stage = nullptr;
@@ -823,7 +823,6 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
     smax_touch(h, level, sout);
     // the combination stage can also reduce the max signal speed of what it writes (a1 fused into a6)
     const bool fuse = h->kernel != 0 && h->fuse_cfl != 0 && a != 0.0;
-    const int zs = (h->zsplit == 1 || (h->zsplit == 2 && 2 * n <= h->num_sms)) ? 1 : 0;
     if (fuse) CUDA_TRY(h, cudaMemsetAsync(h->d_smax + level, 0, sizeof(unsigned long long), h->stream));
     if (h->kernel == 0) {
       k_rk_stage_ref<T, NV><<<dim3(n, NI), 256, 0, h->stream>>>(make_pool<T>(h), sin, sbase, sout, first, T(a), T(b),
@@ -833,14 +832,14 @@ int amrhydro_rk_stage(amrhydro_t *h, int level, int sin, int sbase, int sout, do
       if constexpr (NV == 5) {
         int r = launch_rk_stage_pair<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                             make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                            fuse ? h->d_smax + level : nullptr, zs, dtd, h->d_bneed);
+                                            fuse ? h->d_smax + level : nullptr, h->zsplit, h->num_sms, dtd, h->d_bneed);
         if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_pair: ") + cudaGetErrorString((cudaError_t)r));
         LAUNCH_CHECK(h);
       }
     } else {
       int r = launch_rk_stage_march<T, NV>(h->tmap, make_pool<T>(h), sin, sbase, sout, first, n, T(a), T(b), T(dt / hx),
                                            make_params<T>(h), bflux, h->d_scalars + 1, h->d_desc, h->halo, h->stream,
-                                           fuse ? h->d_smax + level : nullptr, zs, dtd);
+                                           fuse ? h->d_smax + level : nullptr, h->zsplit, h->num_sms, dtd);
       if (r) return fail(h, AMRHYDRO_ECUDA, std::string("rk_stage_march: ") + cudaGetErrorString((cudaError_t)r));
       LAUNCH_CHECK(h);
     }

@@ -425,7 +425,7 @@ template <typename T, int NV, bool BASE>
 __global__ void __launch_bounds__(mk::THREADS, (sizeof(T) == 8 ? (NV == 5 ? AMR_MINB64 : 1) : (NV == 5 ? (BASE && AMR_BASE_TMA ? 2 : AMR_MINB32) : 2)))
 k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin, int sbase, int sout, int first, T a, T b,
                  T dtdx, Params<T> P, T *__restrict__ bflux, unsigned long long *__restrict__ floor_hits,
-                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int zsplit, DtDev dtd) {
+                 const Desc *__restrict__ desc, int direct_halo, unsigned long long *__restrict__ smax_out, int nfull, DtDev dtd) {
   using S = mk::Smem<T, NV, BASE>;
   if (dtd.p) dtdx = T((*dtd.p * dtd.pow2) / dtd.hx);
   constexpr int PW = S::PW, PQ = S::PQ, PY = S::PY, WV = S::WV, QXV = S::QXV, QYV = S::QYV, RAWP = S::RAWP;
@@ -435,9 +435,12 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
   T *sm = reinterpret_cast<T *>(smem_raw + ((128u - (mk::smem_u32(smem_raw) & 127u)) & 127u));
   unsigned long long *bars = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(sm) + S::BAR_OFF);
 
-  // zsplit = 1 (levels too small to fill the machine): two CTAs per patch, each marching over 8 of the 16 cells in z
-  const int pl = blockIdx.x >> zsplit, p = first + pl;
-  const int zlo = int(blockIdx.x & zsplit) * (NI / 2), nz = zsplit ? NI / 2 : NI;
+  // z-split: blocks 0 .. nfull-1 march over a whole patch; the blocks behind them come in pairs, two CTAs per patch, each
+  // marching over 8 of the 16 cells in z (all patches of a level too small to fill the machine: nfull = 0; or the last,
+  // less than half full wave of a launch, which then takes 0.6 instead of 1 wave time).  Bitwise the unsplit march.
+  const bool zhalf = int(blockIdx.x) >= nfull;
+  const int pl = zhalf ? nfull + ((int(blockIdx.x) - nfull) >> 1) : int(blockIdx.x), p = first + pl;
+  const int zlo = zhalf ? ((int(blockIdx.x) - nfull) & 1) * (NI / 2) : 0, nz = zhalf ? NI / 2 : NI;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const T kk = T(0.5) * b * dtdx;        // the 1/2 of Eq. 12 is applied here (G = 2F)
   const T th2 = T(2) * P.theta, q4 = T(0.25);
@@ -674,22 +677,34 @@ int make_tensor_map(CUtensorMap *tm, void *pool_base, size_t max_patches, int ns
 template <typename T, int NV>
 int launch_rk_stage_march(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                           T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
+                          cudaStream_t stream, unsigned long long *smax_out = nullptr, int zmode = 0, int num_sms = 0, DtDev dtd = DtDev{nullptr, 0, 0}) {
   static bool configured = false;
+  static int cps[2] = {1, 1};               // resident CTAs per SM of the two instantiations
   constexpr size_t bytes0 = mk::Smem<T, NV, false>::BYTES, bytes1 = mk::Smem<T, NV, true>::BYTES;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes0));
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(k_rk_stage_march<T, NV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes1));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cps[0], k_rk_stage_march<T, NV, false>, mk::THREADS, bytes0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cps[1], k_rk_stage_march<T, NV, true>, mk::THREADS, bytes1);
     if (e != cudaSuccess) return int(e);
     configured = true;
   }
+  // zmode 0: never split; 1: every patch; 2: every patch of a level of at most num_sms / 2 patches, else the patches of
+  // the last wave of the launch if that wave is less than half full (their half-CTAs then all fit into it)
+  int nfull = n;
+  if (zmode == 1 || (zmode == 2 && 2 * n <= num_sms)) nfull = 0;
+  else if (zmode == 2) {
+    const int slots = std::max(1, cps[a != T(0) ? 1 : 0]) * num_sms, tail = n % slots;
+    if (n > slots && tail > 0 && 2 * tail <= slots) nfull = n - tail;
+  }
+  const int grid = nfull + 2 * (n - nfull);
   if (a != T(0))
-    k_rk_stage_march<T, NV, true><<<n << zsplit, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                                bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd);
+    k_rk_stage_march<T, NV, true><<<grid, mk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                                bflux, floor_hits, desc, direct_halo, smax_out, nfull, dtd);
   else
-    k_rk_stage_march<T, NV, false><<<n << zsplit, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
-                                                                                 bflux, floor_hits, desc, direct_halo, nullptr, zsplit, dtd);
+    k_rk_stage_march<T, NV, false><<<grid, mk::THREADS, bytes0, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
+                                                                                 bflux, floor_hits, desc, direct_halo, nullptr, nfull, dtd);
   return 0;
 }
 

@@ -530,7 +530,7 @@ k_rk_stage_pair(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin,
 template <typename T, int NV>
 int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sbase, int sout, int first, int n, T a, T b,
                          T dtdx, Params<T> P, T *bflux, unsigned long long *floor_hits, const Desc *desc, int direct_halo,
-                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zsplit = 0, DtDev dtd = DtDev{nullptr, 0, 0},
+                         cudaStream_t stream, unsigned long long *smax_out = nullptr, int zmode = 0, int num_sms = 0, DtDev dtd = DtDev{nullptr, 0, 0},
                          const int *bneed = nullptr) {
   static bool configured = false;
   constexpr size_t bytes0 = pk::Smem<T, NV, false>::BYTES, bytes1 = pk::Smem<T, NV, true>::BYTES;
@@ -541,6 +541,10 @@ int launch_rk_stage_pair(const CUtensorMap &tmap, Pool<T> pool, int sin, int sba
     if (e != cudaSuccess) return int(e);
     configured = true;
   }
+  // zmode 0: never split; 1: every patch; 2: every patch of a level of at most num_sms / 2 patches.  (The march kernel also
+  // splits the thin last wave of a launch; here the block decode that takes costs the fp64 instantiation its last free
+  // registers: 16-32 bytes of spills, 10.6 -> 12.8 ms at 512^3.)
+  const int zsplit = (zmode == 1 || (zmode == 2 && 2 * n <= num_sms)) ? 1 : 0;
   if (a != T(0))
     k_rk_stage_pair<T, NV, true><<<n << zsplit, pk::THREADS, bytes1, stream>>>(tmap, pool, sin, sbase, sout, first, a, b, dtdx, P,
                                                                               bflux, floor_hits, desc, direct_halo, smax_out, zsplit, dtd, bneed);
