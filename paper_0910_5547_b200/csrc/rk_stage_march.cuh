@@ -303,7 +303,14 @@ template <typename T, int NV, bool WB = true> struct Smem {   // WB: the kernel 
   static constexpr int O_BRAW = ((O_ACC + 31) / 32) * 32;
   static constexpr bool BTMA = WB && AMR_BASE_TMA && (sizeof(T) == 8 || NV == 5) &&
                                size_t(O_BRAW + NSLOT * RAWP) * sizeof(T) + 256 <= 232448;   // 227 kB per CTA (Euler fits, fp64 GLM-9 does not)
-  static constexpr int O_END = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
+  // fp64 GLM-9: q+ of the cell below (the z state carried from pass to pass) is parked here over the x/y phases, where the
+  // nine variables do not fit into the 168 registers of a 10-warp CTA ([NV][256], one slot per interior thread)
+#ifndef AMR_MK_PARK
+#define AMR_MK_PARK 1
+#endif
+  static constexpr bool PARK = AMR_MK_PARK && sizeof(T) == 8 && NV == 9;
+  static constexpr int O_PARK = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
+  static constexpr int O_END = O_PARK + (PARK ? NV * NI * NI : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
   static constexpr size_t BYTES = BAR_OFF + NSLOT * 8 + 128;   // + slack to align the ring to 128 B
 };
@@ -464,6 +471,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
     T *qx = sm + S::O_QX + j * PQ + i, *fx = sm + S::O_FX + j * PQ + i;   // slot i: q+ of cell i-1 / flux at face i
     T *qy = sm + S::O_QY + j * PY + i, *fy = sm + S::O_FY + j * PY + i;
     T dzm[NV], qpz[NV], acc[NV];
+    T *zpark = sm + S::O_PARK + tid;    // (S::PARK only)
     T best = T(0);                      // fused CFL reduction (a1) over the cells this thread finishes
     bool bad = false;
     // raw plane pk -> primitives of this column in primitive buffer pk & 1
@@ -499,6 +507,7 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
         dzm[v] = Wc[v] - W1[v];
         const T s = mk::slope4(dm, dzm[v], dm + dzm[v], th2);            // (the sum, as in the loop: a z-split march must give the same bits)
         qpz[v] = fma(q4, s, W1[v]);                                 // q+ of the ghost cell below plane 2
+        if (S::PARK) zpark[v * (NI * NI)] = qpz[v];
         acc[v] = T(0);
       }
     }
@@ -534,10 +543,19 @@ k_rk_stage_march(const __grid_constant__ CUtensorMap tmap, Pool<T> pool, int sin
           qp[v] = fma(q4, s, Wc[v]);
           dzm[v] = dp;
         }
+        if (S::PARK) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) qpz[v] = zpark[v * (NI * NI)];
+        }
         mk::floor_states<T, NV>(qpz, qm, P, hits);
         mk::face_flux<T, 2>(qpz, qm, P, Gz);
+        if (S::PARK) {
 #pragma unroll
-        for (int v = 0; v < NV; ++v) qpz[v] = qp[v];
+          for (int v = 0; v < NV; ++v) zpark[v * (NI * NI)] = qp[v];
+        } else {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) qpz[v] = qp[v];
+        }
       }
       if (bflux && ((c - NG + zlo) & 7) == 0) {
         T *B = bflux + ((size_t(pl) * 9 + 6 + ((c - NG + zlo) >> 3)) * NV) * 256 + j * 16 + i;
