@@ -287,7 +287,8 @@ template <> struct Cfg<float> { static constexpr int PW = 26, PQ = 18, PY = 18, 
 template <typename T, int NV, bool WB = true> struct Smem {   // WB: the kernel reads U_base (combination stage)
   static constexpr int PW = Cfg<T>::PW, PQ = Cfg<T>::PQ, PY = Cfg<T>::PY;
   // (the fp64 GLM-9 combination stage takes a ring of three, the minimum, so that its U_base ring fits beside it)
-  static constexpr int NSLOT = (WB && AMR_BASE_TMA && sizeof(T) == 8 && NV == 9) ? 3 : Cfg<T>::NSLOT;
+  // (and the MHD-8 one: 256^3 3.13 -> 3.05 ms per step with 33 kB less shared memory, i.e. more L1 for its 16-24 bytes of spills)
+  static constexpr int NSLOT = (WB && AMR_BASE_TMA && sizeof(T) == 8 && NV >= 8) ? 3 : Cfg<T>::NSLOT;
   static constexpr int RAWP = NV * NI * NI;        // one raw plane: [NV][16][16], dense TMA box
   static constexpr int WV = NP * PW;               // one variable of one primitive plane [20][PW]
   static constexpr int QXV = NI * PQ;              // [16][PQ]: slot s = q+ of cell s-1 / flux at face s
@@ -308,7 +309,7 @@ template <typename T, int NV, bool WB = true> struct Smem {   // WB: the kernel 
 #ifndef AMR_MK_PARK
 #define AMR_MK_PARK 1
 #endif
-  static constexpr bool PARK = AMR_MK_PARK && sizeof(T) == 8 && NV == 9;
+  static constexpr bool PARK = AMR_MK_PARK && sizeof(T) == 8 && NV == 9;   // (MHD-8, which does not spill in stage 1: 3.05 -> 3.37 ms with it)
   static constexpr int O_PARK = O_BRAW + (BTMA ? NSLOT * RAWP : 0);
   static constexpr int O_END = O_PARK + (PARK ? NV * NI * NI : 0);
   static constexpr size_t BAR_OFF = ((size_t(O_END) * sizeof(T) + 15) / 16) * 16;
