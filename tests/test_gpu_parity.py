@@ -261,6 +261,26 @@ def test_rk_stage_zsplit_bitwise_equal(gpu, nv, dtype, halo):
         assert np.array_equal(a, c) and np.array_equal(b, d)
 
 
+@pytest.mark.parametrize("nv,nb", [(8, 6), (9, 6), (5, 6)])
+def test_rk_stage_tail_zsplit_bitwise_equal(gpu, nv, nb):
+    """AMRHYDRO_OPT_ZSPLIT = 2 on a level of several waves: the 8- / 9-variable kernel (one CTA per SM) marches the patches
+    of a thin last wave as half-patch CTAs in the same launch (216 patches = 1.46 waves of 148: 68 patches are split).
+    Bitwise the unsplit march, the fused maximum signal speed included; the 5-variable kernel does not split here."""
+    import torch
+    if torch.cuda.get_device_properties(0).multi_processor_count >= 6 ** 3:
+        pytest.skip("the level fits one wave on this device")
+    h = wl.uniform_hierarchy(nb, periodic=True)
+    U = rand_state(h, nv, 77, 5.0 / 3.0)
+    out = []
+    for zs in (0, 2):
+        g = gpu.AmrHydro(h, 5.0 / 3.0, nv, zsplit=zs)
+        g.upload(0, U)
+        dts = [g.advance(0.3) for _ in range(2)]
+        out.append((g.download(0), dts))
+    assert np.isfinite(out[0][0]).all() and not np.array_equal(out[0][0], U)
+    assert np.array_equal(out[0][0], out[1][0]) and out[0][1] == out[1][1]
+
+
 def test_rk_stage_outflow_and_tile_vs_reference_kernel(gpu):
     h = wl.uniform_hierarchy(2, periodic=False)
     U = rand_state(h, 5, 8)
