@@ -57,6 +57,8 @@ def parse():
     ap.add_argument("--zsplit", type=int, default=2, help="AMRHYDRO_OPT_ZSPLIT (2 = automatic)")
     ap.add_argument("--fuse-cfl", type=int, default=2, help="AMRHYDRO_OPT_FUSE_CFL (2 = library default)")
     ap.add_argument("--graph", type=int, default=1, help="AMRHYDRO_OPT_GRAPH for the AMR workload (cfg3): one CUDA-graph replay per coarse step")
+    ap.add_argument("--order", default="zstrip", help="patch order of the single-level workloads: zstrip (strips of 8 rows, z outermost: "
+                    "sibling halos hit in L2), morton, linear")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-fp32", action="store_true", help="skip the fp32 sub-record of the default fp64 run (cfg5, cfg2)")
@@ -73,7 +75,7 @@ WORKLOADS = {
 }
 
 
-def make_workload(name, size, seed_shift=0):
+def make_workload(name, size, seed_shift=0, order="zstrip"):
     """Returns (hierarchy, U[npatch][nv][16][16][16] float64, cell-updates per coarse step)."""
     w = WORKLOADS[name]
     n = size or w["size"]
@@ -87,7 +89,7 @@ def make_workload(name, size, seed_shift=0):
         U = wl.sedov_hierarchy_state(h, gamma=w["gamma"])
         upd = sum(int((h["level"] == l).sum()) * 4096 * (1 << l) for l in range(h["nlevels"]))
         return h, U, upd
-    h = wl.uniform_hierarchy(n // 16, periodic=True)
+    h = wl.uniform_hierarchy(n // 16, periodic=True, order=order)
     if name == "cfg5":
         G = wl.stress_global(n, gamma=w["gamma"], seed=20005 + seed_shift)
     elif name == "cfg2":
@@ -240,7 +242,7 @@ def run_ours(args):
 
     w = WORKLOADS[args.workload]
     nv, gamma, cfl = w["nv"], w["gamma"], w["cfl"]
-    h, U, upd_per_step = make_workload(args.workload, args.size, seed_shift=rank)
+    h, U, upd_per_step = make_workload(args.workload, args.size, seed_shift=rank, order=args.order)
     npatch = len(h["level"])
     single = h["nlevels"] == 1
     esz = 8 if args.dtype == "f64" else 4
@@ -399,6 +401,7 @@ def run_ours(args):
             "config": {"workload": w["name"] if not args.size or args.size == w["size"] else
                        w["name"] + " (REDUCED to %d cells per side by --size)" % args.size, "patches": npatch, "cells": npatch * 4096, "nvars": nv,
                        "cfl": cfl, "halo": "direct sibling reads" if args.halo else "materialised ghosts",
+                       "patch_order": "criterion-built table (Morton)" if args.workload == "cfg3" else args.order,
                        "l2_policy": "working set (%.1f GB per slot) far exceeds the 126 MB L2" % (npatch * nv * 4096 * esz / 1e9)
                        if npatch * nv * 4096 * esz > 4 * 126e6 else "working set fits L2 (small config)",
                        "parallelism": "replicas, one per GPU" if world > 1 else "single GPU",

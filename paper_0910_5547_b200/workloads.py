@@ -19,6 +19,9 @@ BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
 # --------------------------------------------------------------------------- hierarchy
+ZSTRIP_ROWS = 8      # 32 x 8 patches per z-layer of a strip at 512^3: one wave of the fp64 stage kernel (296 CTAs)
+
+
 def _morton(b):
     key = 0
     for bit in range(10):
@@ -46,6 +49,17 @@ def build_hierarchy(base_blocks, refined=(), bc=(0,) * 6, box=1.0, order="morton
         levels.append(sorted(set(tuple(int(x) for x in b) for b in blocks)))
     if order == "morton":
         levels = [sorted(lv, key=_morton) for lv in levels]
+    elif order == "zstrip":
+        # launch order for large single-level runs (any order is a valid table): strips of ZSTRIP_ROWS rows of patches in
+        # y; inside a strip z outermost, then y, then x.  One wave of CTAs is then about one z-layer of a strip: x and y
+        # neighbours march in step and a patch starts roughly one wave after the patch below it, when that one has just
+        # read the planes the two share -- the sibling-halo reads hit in L2 instead of DRAM
+        def key(b, l):
+            nx, nz = base_blocks[0] << l, base_blocks[2] << l
+            return ((b[1] // ZSTRIP_ROWS) * nz + b[2]) * (ZSTRIP_ROWS * nx) + (b[1] % ZSTRIP_ROWS) * nx + b[0]
+        levels = [sorted(lv, key=lambda b, l=l: key(b, l)) for l, lv in enumerate(levels)]
+    elif order != "linear":
+        raise ValueError("order must be morton, zstrip or linear")
     ids, pid = [], 0
     for lv in levels:
         m = {}

@@ -129,3 +129,29 @@ def test_partitioner_properties():
         sharding.partition_morton(wl.ball_hierarchy(2, 2), 2)
     with pytest.raises(ValueError):
         sharding.partition_morton(h, 65)
+
+
+def test_zstrip_table_order_is_consistent():
+    """workloads.build_hierarchy(order="zstrip"): the launch order of the single-level bench workloads.  Any order is a valid
+    table; check the neighbour entries against the block coordinates and the order itself (strips of 8 rows, z outermost)."""
+    import numpy as np
+    from paper_0910_5547_b200 import workloads as wl
+    nb = (6, 16, 4)
+    h = wl.build_hierarchy(nb, (), (0,) * 6, order="zstrip")
+    B = np.asarray(h["blocks"]); n = len(B)
+    assert n == 6 * 16 * 4 and len({tuple(b) for b in B}) == n
+    index = {tuple(int(c) for c in b): i for i, b in enumerate(B)}
+    for i in (0, 17, n // 2, n - 1):
+        for r in range(27):
+            d = (r % 3 - 1, (r // 3) % 3 - 1, r // 9 - 1)
+            q = tuple((int(B[i][a]) + d[a]) % nb[a] for a in range(3))
+            assert h["nbr"][i][r] == index[q]
+    key = [((b[1] // wl.ZSTRIP_ROWS) * nb[2] + b[2], b[1] % wl.ZSTRIP_ROWS, b[0]) for b in B]
+    assert key == sorted(key)
+    assert [tuple(b) for b in B[:7]] == [(0, 0, 0), (1, 0, 0), (2, 0, 0), (3, 0, 0), (4, 0, 0), (5, 0, 0), (0, 1, 0)]
+    assert tuple(B[6 * wl.ZSTRIP_ROWS]) == (0, 0, 1)                     # after one z-layer of the first strip: up in z
+    try:
+        wl.build_hierarchy(nb, (), (0,) * 6, order="spiral")
+        assert False
+    except ValueError:
+        pass
