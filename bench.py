@@ -12,11 +12,14 @@ e2e (host buffers through amrhydro_advance_host), roofline of the stage kernel (
 bytes / CUDA-event time / measured HBM peak, plus the ncu DRAM bytes and the issue / FP64-pipe
 fractions), cpu_baseline (the oracle on the host cores), clocks (NVML samples in the timed region).
 --workload cfg3 (AMR) runs amrhydro_advance as one CUDA-graph replay per coarse step.
+Single-level workloads are built in the "zstrip" table order (--order; workloads.build_hierarchy): the launch order in
+which sibling halos hit in L2 (real DRAM traffic 1.2x instead of 1.44x the algorithmic bytes; any order gives the same bits).
 --gpus N (torchrun): N independent replicas, weak scaling, max-over-ranks timing.
 --impl reference: the CPU oracle on a bounded sample (there is no reference implementation).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--impl ours|reference]
                   [--workload cfg5|cfg2|cfg4|cfg4g|cfg3] [--size S] [--halo 0|1] [--graph 0|1] [--no-fp32]
+                  [--order zstrip|morton|linear]
 """
 import argparse
 import json
